@@ -1,0 +1,200 @@
+"""fp64 CPU oracle for the e3j hot path -- TEST INFRASTRUCTURE ONLY.
+
+Thin ctypes marshalling over ``oracle/e3_oracle.c`` (plain C, double precision, the
+definitions of SURVEY.md section 8(c); see the header of that file for citations and pins).
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this module.  It imports nothing from the CUDA
+package ``paper_2605_22698_b200`` and the CUDA package never imports it.
+
+Every array crossing this boundary is float64 / int32 numpy, C-contiguous.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "e3_oracle.c")
+_LIB = os.path.join(_HERE, "libe3_oracle.so")
+
+
+def build(force: bool = False) -> str:
+    """Compile the C oracle with gcc (-O2, no fast-math).  Building the checker is not using it."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", _SRC, "-o", _LIB, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+class _Irrep(C.Structure):
+    _fields_ = [("l", C.c_int), ("parity", C.c_int), ("mul", C.c_int)]
+
+
+class _Path(C.Structure):
+    _fields_ = [("i_in", C.c_int), ("l_sh", C.c_int), ("i_out", C.c_int)]
+
+
+_lib = None
+
+
+def _L():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_cg_complex.restype = C.c_double
+        _lib.orc_cg_complex.argtypes = [C.c_int] * 6
+        _lib.orc_cg_real.restype = C.c_double
+        _lib.orc_num_threads.restype = C.c_int
+    return _lib
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _plan_args(irreps_in, sh_lmax, irreps_out, paths):
+    """irreps_*: sequence of (l, parity(+1/-1), mul); paths: sequence of (i_in, l_sh, i_out)."""
+    ii = (_Irrep * len(irreps_in))(*[_Irrep(*map(int, t)) for t in irreps_in])
+    io = (_Irrep * len(irreps_out))(*[_Irrep(*map(int, t)) for t in irreps_out])
+    pp = (_Path * len(paths))(*[_Path(*map(int, t)) for t in paths])
+    return (ii, C.c_int(len(irreps_in)), C.c_int(int(sh_lmax)), io, C.c_int(len(irreps_out)), pp, C.c_int(len(paths)))
+
+
+def num_threads() -> int:
+    return int(_L().orc_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    _L().orc_set_num_threads(C.c_int(int(n)))
+
+
+def cg_complex(l1, m1, l2, m2, l3, m3) -> float:
+    """Condon-Shortley <l1 m1 l2 m2 | l3 m3> (Racah closed form)."""
+    return float(_L().orc_cg_complex(l1, m1, l2, m2, l3, m3))
+
+
+def cg_real(l1, l2, l3, return_discarded=False):
+    """Dense real CG tensor [(2l1+1),(2l2+1),(2l3+1)] (reading A4)."""
+    out = np.zeros((2 * l1 + 1, 2 * l2 + 1, 2 * l3 + 1), dtype=np.float64)
+    d = _L().orc_cg_real(C.c_int(l1), C.c_int(l2), C.c_int(l3), _p(out))
+    return (out, float(d)) if return_discarded else out
+
+
+def sh(lmax, vec):
+    """Y[n,(lmax+1)^2] of raw vectors vec[n,3] (component normalisation, readings A1-A3)."""
+    vec = _f64(vec).reshape(-1, 3)
+    Y = np.empty((vec.shape[0], (lmax + 1) ** 2), dtype=np.float64)
+    _L().orc_sh(C.c_int(lmax), C.c_int64(vec.shape[0]), _p(vec), _p(Y))
+    return Y
+
+
+def sh_jac(lmax, vec):
+    """J[n,(lmax+1)^2,3] = dY/dvec."""
+    vec = _f64(vec).reshape(-1, 3)
+    J = np.empty((vec.shape[0], (lmax + 1) ** 2, 3), dtype=np.float64)
+    _L().orc_sh_jac(C.c_int(lmax), C.c_int64(vec.shape[0]), _p(vec), _p(J))
+    return J
+
+
+def sh_bwd(lmax, vec, dY):
+    vec = _f64(vec).reshape(-1, 3)
+    dY = _f64(dY)
+    dvec = np.empty_like(vec)
+    _L().orc_sh_bwd(C.c_int(lmax), C.c_int64(vec.shape[0]), _p(vec), _p(dY), _p(dvec))
+    return dvec
+
+
+def graph_prepare(senders, receivers, n_nodes):
+    senders, receivers = _i32(senders), _i32(receivers)
+    E = senders.shape[0]
+    row_ptr = np.empty(n_nodes + 1, dtype=np.int32)
+    col_ptr = np.empty(n_nodes + 1, dtype=np.int32)
+    perm_s = np.empty(E, dtype=np.int32)
+    rc = _L().orc_graph_prepare(_p(senders), _p(receivers), C.c_int64(E), C.c_int32(n_nodes),
+                                _p(row_ptr), _p(perm_s), _p(col_ptr))
+    if rc:
+        raise ValueError("oracle graph_prepare: index out of range")
+    return row_ptr, perm_s, col_ptr
+
+
+def plan_dims(irreps_in, sh_lmax, irreps_out, paths):
+    a = _plan_args(irreps_in, sh_lmax, irreps_out, paths)
+    i, s, o = C.c_int(), C.c_int(), C.c_int()
+    rc = _L().orc_plan_dims(*a, C.byref(i), C.byref(s), C.byref(o))
+    if rc:
+        raise ValueError(f"oracle plan invalid (code {rc})")
+    return i.value, s.value, o.value
+
+
+def tp_scatter_fwd(irreps_in, sh_lmax, irreps_out, paths, x, Y, w, senders, receivers, n_nodes):
+    """out[N, out_dim*C] -- SURVEY 8(a) a4, dense definition."""
+    a = _plan_args(irreps_in, sh_lmax, irreps_out, paths)
+    in_dim, sh_dim, out_dim = plan_dims(irreps_in, sh_lmax, irreps_out, paths)
+    Cm = int(irreps_in[0][2])
+    x, Y, w = _f64(x), _f64(Y), _f64(w)
+    senders, receivers = _i32(senders), _i32(receivers)
+    E = senders.shape[0]
+    assert x.size == n_nodes * in_dim * Cm and Y.size == E * sh_dim and w.size == E * len(paths) * Cm
+    out = np.empty((n_nodes, out_dim * Cm), dtype=np.float64)
+    rc = _L().orc_tp_scatter_fwd(*a, _p(x), _p(Y), _p(w), _p(senders), _p(receivers),
+                                 C.c_int64(E), C.c_int32(n_nodes), _p(out))
+    if rc:
+        raise ValueError(f"oracle plan invalid (code {rc})")
+    return out
+
+
+def tp_scatter_bwd(irreps_in, sh_lmax, irreps_out, paths, x, Y, w, senders, receivers, n_nodes, g):
+    """(dx[N,in_dim*C], dY[E,sh_dim], dw[E,P*C]) -- SURVEY 8(a) a5, dense definition."""
+    a = _plan_args(irreps_in, sh_lmax, irreps_out, paths)
+    in_dim, sh_dim, out_dim = plan_dims(irreps_in, sh_lmax, irreps_out, paths)
+    Cm = int(irreps_in[0][2])
+    x, Y, w, g = _f64(x), _f64(Y), _f64(w), _f64(g)
+    senders, receivers = _i32(senders), _i32(receivers)
+    E = senders.shape[0]
+    assert g.size == n_nodes * out_dim * Cm
+    dx = np.empty((n_nodes, in_dim * Cm), dtype=np.float64)
+    dY = np.empty((E, sh_dim), dtype=np.float64)
+    dw = np.empty((E, len(paths) * Cm), dtype=np.float64)
+    rc = _L().orc_tp_scatter_bwd(*a, _p(x), _p(Y), _p(w), _p(senders), _p(receivers),
+                                 C.c_int64(E), C.c_int32(n_nodes), _p(g), _p(dx), _p(dY), _p(dw))
+    if rc:
+        raise ValueError(f"oracle plan invalid (code {rc})")
+    return dx, dY, dw
+
+
+def force_reduce(dvec, senders, receivers, n_nodes):
+    dvec = _f64(dvec).reshape(-1, 3)
+    senders, receivers = _i32(senders), _i32(receivers)
+    F = np.empty((n_nodes, 3), dtype=np.float64)
+    _L().orc_force_reduce(_p(dvec), _p(senders), _p(receivers), C.c_int64(dvec.shape[0]), C.c_int32(n_nodes), _p(F))
+    return F
+
+
+def all_paths(irreps_in, sh_lmax, out_lmax, natural_parity_only=False):
+    """Benchmark path table (reading A5/A6), the oracle's own enumerator.
+
+    irreps_in: sequence of (l, parity, mul).  Every (i_in, l2 <= sh_lmax, l3) with
+    |l1-l2| <= l3 <= min(l1+l2, out_lmax); output parity p1 * (-1)^l2 (pseudotensor outputs
+    included unless natural_parity_only); order i_in, then l2, then l3 ascending; each path
+    gets its own output block.  Returns (irreps_out, paths)."""
+    irreps_out, paths = [], []
+    for i_in, (l1, p1, mul) in enumerate(irreps_in):
+        for l2 in range(sh_lmax + 1):
+            for l3 in range(abs(l1 - l2), min(l1 + l2, out_lmax) + 1):
+                p3 = p1 * (-1) ** l2
+                if natural_parity_only and p3 != (-1) ** l3:
+                    continue
+                irreps_out.append((l3, p3, mul))
+                paths.append((i_in, l2, len(irreps_out) - 1))
+    return irreps_out, paths
