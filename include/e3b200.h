@@ -1,0 +1,185 @@
+/*
+ * e3b200.h -- C ABI of the B200-native fused Clebsch-Gordan tensor product + scatter library
+ * (the data-parallel hot path of the e3j backend of arxiv 2605.22698, "mlip v2").
+ *
+ * The paper only NAMES the operation: PAPER.md L72-L74 (section 4: MACE and NequIP "rely on the
+ * Clebsch-Gordan Tensor Product ... a significant computational bottleneck"), L82 ("fusion of
+ * the message passing kernel" is the authors' open item), L66 (the Graph class computes edge
+ * vectors from positions and connectivity), L44 (CG formalism).  It prints no formula, so every
+ * convention below is a reading fixed in SURVEY.md section 8(c) / DESIGN.md (A1..A18); each
+ * entry point cites the reading that defines what it computes.
+ *
+ * General rules
+ *  - Plain C types only.  Every pointer is a DEVICE pointer owned by the caller unless its
+ *    name ends in _h / it is documented as host.  The library never frees or keeps caller
+ *    memory, never allocates on the hot path, and launches only on the given stream.
+ *  - `e3_stream` is a cudaStream_t passed as an opaque pointer (NULL = legacy default stream).
+ *  - No call synchronises the stream except where stated (e3_graph_prepare with validate != 0,
+ *    e3_plan_create, the e3_session_* host-buffer calls).
+ *  - Every function returns an int status (E3_OK == 0).  e3_last_error() returns a
+ *    thread-local detail string (NVRTC log, CUDA error text) for the last failing call.
+ *  - Layouts (reading A7): a node row is the concatenation of its irrep blocks in irreps order;
+ *    inside a block the element index is m*C + u, m = 0..2l (i.e. m_true + l), u = channel
+ *    (channel fastest).  SH rows are indexed l*l + l + m_true.  Weights are [(e*P + p)*C + u]
+ *    (64-bit offsets).  All irreps of a plan share one multiplicity C ("uvu", reading A8).
+ *  - dtype (reading A12): E3_F32 stores feats, sh, weights and grad_weights as float;
+ *    E3_BF16 stores those four as bfloat16 (round-to-nearest-even) and everything else
+ *    (out, grad_out, grad_feats, grad_sh, vec, grad_vec, forces, accumulators) as float.
+ *  - There is no CPU fallback anywhere: without a CUDA device every compute call returns
+ *    E3_ERR_CUDA.
+ */
+#ifndef E3B200_H
+#define E3B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct e3_plan e3_plan;          /* opaque, immutable after creation, thread-safe for launches */
+typedef struct e3_session e3_session;    /* opaque, owns device buffers for the host-buffer entry point */
+typedef void *e3_stream;                 /* cudaStream_t */
+
+typedef struct { int l; int parity; /* +1 even, -1 odd */ int mul; } e3_irrep;
+typedef struct { int i_in; int l_sh; int i_out; } e3_path;   /* indices into irreps_in / irreps_out */
+typedef enum { E3_F32 = 0, E3_BF16 = 1 } e3_dtype;
+
+enum {
+    E3_OK = 0,
+    E3_ERR_INVALID_ARG = 1,   /* null pointer, negative size, index out of range                     */
+    E3_ERR_BAD_PATH = 2,      /* triangle rule, parity rule or irrep index violated                  */
+    E3_ERR_UNSUPPORTED = 3,   /* l > 3, unequal multiplicities, C*dtype row not 4-byte aligned, ...  */
+    E3_ERR_UNSORTED = 4,      /* receivers not ascending (only when validation was requested)        */
+    E3_ERR_CUDA = 5,          /* CUDA runtime error or no device                                     */
+    E3_ERR_JIT = 6,           /* run-time specialisation (NVRTC) of the plan's kernels failed        */
+    E3_ERR_WORKSPACE = 7      /* workspace pointer NULL or too small                                 */
+};
+
+const char *e3_status_string(int status);
+const char *e3_last_error(void);
+
+/* ---------------------------------------------------------------------------------------------
+ * Path table helper (host only).  Reading A5/A6: every (i_in, l2 <= sh_lmax, l3) with
+ * |l1-l2| <= l3 <= min(l1+l2, out_lmax), output parity p1*(-1)^l2 (pseudotensor outputs included
+ * unless natural_parity_only), ordered by i_in, then l2, then l3; each path gets its own output
+ * irrep (multiplicity of its input).  Call with out == NULL / paths == NULL to query the counts.
+ * -------------------------------------------------------------------------------------------*/
+int e3_all_paths(const e3_irrep *irreps_in, int n_in, int sh_lmax, int out_lmax, int natural_parity_only,
+                 e3_irrep *irreps_out, int *n_out, e3_path *paths, int *n_paths);
+
+/* ---------------------------------------------------------------------------------------------
+ * Plan.  Validates the path table (E3_ERR_BAD_PATH), computes the real
+ * Clebsch-Gordan tensors of all paths ON THE DEVICE in fp64 (Racah closed form + real-basis
+ * change, reading A4), compacts them to sparse (m1,m2,m3,coef) lists and specialises the
+ * forward and VJP kernels for this plan (coefficients become FFMA immediates).  Needs a device;
+ * synchronises; takes O(seconds) once.  A path whose i_out is shared with another path ADDS
+ * into that block (A6).  Limits: l <= 3 everywhere, all multiplicities equal.
+ * -------------------------------------------------------------------------------------------*/
+int e3_plan_create(e3_plan **plan, const e3_irrep *irreps_in, int n_in, int sh_lmax,
+                   const e3_irrep *irreps_out, int n_out, const e3_path *paths, int n_paths, e3_dtype dtype);
+int e3_plan_destroy(e3_plan *plan);
+/* in_dim = sum(2l+1) over irreps_in, sh_dim = (sh_lmax+1)^2, out_dim likewise over irreps_out,
+ * weights_per_edge = n_paths * C, nnz_total = number of non-zero real CG coefficients. */
+int e3_plan_dims(const e3_plan *plan, int *in_dim, int *sh_dim, int *out_dim, int *weights_per_edge, int *nnz_total);
+/* Host copy of path `path`'s sparse CG list (m indices are 0-based: m_true + l).  Pass m1 == NULL
+ * to query *nnz only.  Order: m1, then m2, then m3 ascending. */
+int e3_plan_get_cg(const e3_plan *plan, int path, int *m1, int *m2, int *m3, double *coef, int *nnz);
+/* Launch facts of the specialised kernels: which = 0 forward, 1 backward.  Any pointer may be NULL. */
+int e3_plan_kernel_info(const e3_plan *plan, int which, int *regs, int *spill_bytes, int *smem_bytes,
+                        int *threads_per_block, int *n_roles, int *channels_per_lane);
+/* Algorithmic work per edge of this plan, SURVEY 8(d) formulas (factored form), for roofline reports. */
+int e3_plan_work(const e3_plan *plan, double *fwd_flop_per_edge, double *bwd_flop_per_edge);
+
+/* Build-time check (host only, no device needed): generates and compiles the specialised
+ * kernels exactly as e3_plan_create would, using a host evaluation of the same CG routine, and
+ * reports registers / spills.  If src_path != NULL the generated CUDA source is written there
+ * and the cubin beside it (src_path + ".cubin").  It computes nothing of the hot path. */
+int e3_jit_check(const e3_irrep *irreps_in, int n_in, int sh_lmax, const e3_irrep *irreps_out, int n_out,
+                 const e3_path *paths, int n_paths, e3_dtype dtype, const char *src_path,
+                 int *fwd_regs, int *fwd_spill, int *bwd_regs, int *bwd_spill);
+
+/* ---------------------------------------------------------------------------------------------
+ * Graph preparation (readings A11/A14/A15).  Integer only, deterministic.
+ * Input: receivers ascending.  Output: row_ptr[N+1] (CSR over receivers), perm_s[E] (edge ids in
+ * ascending sender order, ties in ascending edge id = numpy stable argsort), col_ptr[N+1].
+ * workspace: >= e3_graph_workspace_bytes(E, N) bytes of device memory.
+ * validate != 0: additionally checks index ranges and sortedness; this SYNCHRONISES the stream
+ * and returns E3_ERR_INVALID_ARG / E3_ERR_UNSORTED.
+ * -------------------------------------------------------------------------------------------*/
+size_t e3_graph_workspace_bytes(int64_t n_edges, int32_t n_nodes);
+int e3_graph_prepare(const int32_t *senders, const int32_t *receivers, int64_t n_edges, int32_t n_nodes,
+                     int32_t *row_ptr, int32_t *perm_s, int32_t *col_ptr,
+                     void *workspace, size_t workspace_bytes, int validate, e3_stream stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Spherical harmonics (readings A1-A3).  sh[e, l*l+l+m] = Y_lm(vec_e/|vec_e|),
+ * real basis, z polar, m<0 sine / m>0 cosine type, no Condon-Shortley sign, component
+ * normalisation (sum_m Y_lm^2 = 2l+1): Y_1 = sqrt3 (y,z,x).  |vec| == 0 -> Y_00 = 1, rest 0,
+ * gradient 0.  sh has the plan's storage dtype; grad_sh and grad_vec are float.
+ *   grad_vec[e,:] = sum_lm grad_sh[e,lm] * d Y_lm(vec/|vec|) / d vec .
+ * -------------------------------------------------------------------------------------------*/
+int e3_sh_fwd(const e3_plan *plan, const float *vec /*[E,3]*/, int64_t n_edges, void *sh /*[E,sh_dim]*/,
+              e3_stream stream);
+int e3_sh_bwd(const e3_plan *plan, const float *vec, const float *grad_sh /*[E,sh_dim]*/, int64_t n_edges,
+              float *grad_vec /*[E,3]*/, e3_stream stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Fused gather - tensor product - scatter, forward (readings A4-A8, A10):
+ *   out[r, blk(p), m3, u] = sum_{e : receivers[e] = r} weights[e,p,u] *
+ *        sum_{m1,m2} C^p[m1,m2,m3] * feats[senders[e], blk(l1(p)), m1, u] * sh[e, l2(p), m2]
+ * Edges must be sorted by receiver; row_ptr from e3_graph_prepare.  Every row of out[N, out_dim*C]
+ * is written (zeros for receivers without edges).  Deterministic: each (receiver, output row,
+ * channel) is accumulated by one thread in ascending edge order; no atomics.
+ * `receivers` is accepted for symmetry with the problem statement and may be NULL.
+ * -------------------------------------------------------------------------------------------*/
+int e3_tp_scatter_fwd(const e3_plan *plan, const void *feats /*[N,in_dim*C]*/, const void *sh /*[E,sh_dim]*/,
+                      const void *weights /*[E,P*C]*/, const int32_t *senders, const int32_t *receivers,
+                      const int32_t *row_ptr, int64_t n_edges, int32_t n_nodes, float *out, e3_stream stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * VJP of the forward.  Given grad_out = dL/d out [N, out_dim*C] (float):
+ *   grad_feats[s,l1,m1,u] = sum_{e : senders[e] = s} sum_p w[e,p,u] sum_{m2,m3} C^p sh[e,l2,m2] grad_out[r,p,m3,u]
+ *   grad_sh[e,l2,m2]      = sum_p sum_u w[e,p,u] sum_{m1,m3} C^p feats[s,l1,m1,u] grad_out[r,p,m3,u]
+ *   grad_weights[e,p,u]   = sum_{m1,m2,m3} C^p feats[s,l1,m1,u] sh[e,l2,m2] grad_out[r,p,m3,u]
+ * grad_feats [N,in_dim*C] and grad_sh [E,sh_dim] are float; grad_weights has the plan's storage
+ * dtype and may be NULL (skipped).  workspace: >= e3_bwd_workspace_bytes(plan, E, N) bytes; it
+ * holds the per-edge grad_feats contributions that the second phase sums per sender in
+ * ascending edge order (deterministic, no atomics).
+ * -------------------------------------------------------------------------------------------*/
+size_t e3_bwd_workspace_bytes(const e3_plan *plan, int64_t n_edges, int32_t n_nodes);
+int e3_tp_scatter_bwd(const e3_plan *plan, const void *feats, const void *sh, const void *weights,
+                      const int32_t *senders, const int32_t *receivers, const int32_t *row_ptr,
+                      const int32_t *perm_s, const int32_t *col_ptr, int64_t n_edges, int32_t n_nodes,
+                      const float *grad_out, float *grad_feats, float *grad_sh, void *grad_weights,
+                      void *workspace, size_t workspace_bytes, e3_stream stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Edge -> atom force reduction (reading A10: vec_e = pos[rcv] - pos[snd] + shift):
+ *   forces[i,:] = -( sum_{e : receivers[e]=i} grad_vec[e,:] - sum_{e : senders[e]=i} grad_vec[e,:] )
+ * Fixed summation order (one warp per atom, no atomics).
+ * -------------------------------------------------------------------------------------------*/
+int e3_force_reduce(const float *grad_vec /*[E,3]*/, const int32_t *row_ptr, const int32_t *perm_s,
+                    const int32_t *col_ptr, int64_t n_edges, int32_t n_nodes, float *forces /*[N,3]*/,
+                    e3_stream stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Host-buffer entry point: one pass of the whole hot path (a2..a7) with HOST inputs and outputs.
+ * The session owns device buffers sized for (max_edges, max_nodes) and one stream; each run copies
+ * the inputs host->device, runs graph_prepare, sh_fwd, tp_scatter_fwd, tp_scatter_bwd, sh_bwd and
+ * force_reduce, copies the requested results device->host and synchronises.  Any output pointer
+ * may be NULL (skipped, and its copy is not made).  Inputs have the plan's storage dtype where
+ * the device entry points do.  bytes_h2d / bytes_d2h (may be NULL) receive the bytes copied.
+ * -------------------------------------------------------------------------------------------*/
+int e3_session_create(e3_session **session, const e3_plan *plan, int64_t max_edges, int32_t max_nodes);
+int e3_session_destroy(e3_session *session);
+int e3_session_run_host(e3_session *session, const float *vec_h, const void *feats_h, const void *weights_h,
+                        const int32_t *senders_h, const int32_t *receivers_h, int64_t n_edges, int32_t n_nodes,
+                        const float *grad_out_h, float *out_h, float *grad_feats_h, void *grad_weights_h,
+                        float *grad_vec_h, float *forces_h, int64_t *bytes_h2d, int64_t *bytes_d2h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* E3B200_H */

@@ -1,0 +1,347 @@
+// C ABI entry points (include/e3b200.h): argument checking, launches, the host-buffer session.
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "e3_internal.h"
+
+using namespace e3;
+
+static inline cudaStream_t S(e3_stream s) { return reinterpret_cast<cudaStream_t>(s); }
+static inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+static inline size_t esize(const e3_plan *pl) { return pl->dtype == E3_BF16 ? 2 : 4; }
+
+extern "C" const char *e3_status_string(int status)
+{
+    switch (status) {
+    case E3_OK: return "ok";
+    case E3_ERR_INVALID_ARG: return "invalid argument";
+    case E3_ERR_BAD_PATH: return "path violates triangle/parity/index rule";
+    case E3_ERR_UNSUPPORTED: return "unsupported configuration";
+    case E3_ERR_UNSORTED: return "receivers not sorted";
+    case E3_ERR_CUDA: return "CUDA error or no device";
+    case E3_ERR_JIT: return "kernel specialisation failed";
+    case E3_ERR_WORKSPACE: return "workspace missing or too small";
+    default: return "unknown status";
+    }
+}
+
+extern "C" const char *e3_last_error(void) { return get_error(); }
+
+// ---------------------------------------------------------------------------------------------
+// plan
+// ---------------------------------------------------------------------------------------------
+static int plan_generate(e3_plan &pl, const char *src_path)
+{
+    plan_make_roles(pl);
+    pl.fwd.name = "e3_fwd";
+    pl.bwd.name = "e3_bwd";
+    pl.fwd.source = gen_forward_source(pl);
+    pl.bwd.source = gen_backward_source(pl);
+    pl.fwd.threads = pl.fwd_warps * 32;
+    pl.bwd.threads = pl.bwd_warps * 32;
+    std::string f1, f2;
+    if (src_path) { f1 = std::string(src_path) + ".fwd.cu"; f2 = std::string(src_path) + ".bwd.cu"; }
+    int rc = jit_compile(pl.fwd, f1);
+    if (rc != E3_OK) return rc;
+    return jit_compile(pl.bwd, f2);
+}
+
+extern "C" int e3_plan_create(e3_plan **plan, const e3_irrep *irreps_in, int n_in, int sh_lmax, const e3_irrep *irreps_out,
+                              int n_out, const e3_path *paths, int n_paths, e3_dtype dtype)
+{
+    if (!plan) { set_error("e3_plan_create: plan is NULL"); return E3_ERR_INVALID_ARG; }
+    *plan = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        set_error("e3_plan_create: no CUDA device (this library has no CPU fallback)");
+        return E3_ERR_CUDA;
+    }
+    e3_plan *pl = new (std::nothrow) e3_plan();
+    if (!pl) { set_error("out of host memory"); return E3_ERR_INVALID_ARG; }
+    int rc = plan_build_tables(*pl, irreps_in, n_in, sh_lmax, irreps_out, n_out, paths, n_paths, dtype, /*cg_on_device=*/true);
+    if (rc == E3_OK) rc = plan_generate(*pl, nullptr);
+    if (rc == E3_OK) rc = jit_load(pl->fwd);
+    if (rc == E3_OK) rc = jit_load(pl->bwd);
+    if (rc != E3_OK) { jit_unload(pl->fwd); jit_unload(pl->bwd); delete pl; return rc; }
+    *plan = pl;
+    return E3_OK;
+}
+
+extern "C" int e3_plan_destroy(e3_plan *plan)
+{
+    if (!plan) return E3_OK;
+    jit_unload(plan->fwd);
+    jit_unload(plan->bwd);
+    delete plan;
+    return E3_OK;
+}
+
+extern "C" int e3_plan_dims(const e3_plan *plan, int *in_dim, int *sh_dim, int *out_dim, int *weights_per_edge, int *nnz_total)
+{
+    if (!plan) { set_error("plan is NULL"); return E3_ERR_INVALID_ARG; }
+    if (in_dim) *in_dim = plan->in_dim;
+    if (sh_dim) *sh_dim = plan->sh_dim;
+    if (out_dim) *out_dim = plan->out_dim;
+    if (weights_per_edge) *weights_per_edge = (int)plan->paths.size() * plan->C;
+    if (nnz_total) *nnz_total = plan->nnz_total;
+    return E3_OK;
+}
+
+extern "C" int e3_plan_get_cg(const e3_plan *plan, int path, int *m1, int *m2, int *m3, double *coef, int *nnz)
+{
+    if (!plan || !nnz || path < 0 || path >= (int)plan->paths.size()) { set_error("e3_plan_get_cg: bad arguments"); return E3_ERR_INVALID_ARG; }
+    const PathInfo &pi = plan->paths[path];
+    *nnz = (int)pi.nz.size();
+    if (m1 && m2 && m3 && coef)
+        for (size_t i = 0; i < pi.nz.size(); ++i) { m1[i] = pi.nz[i].m1; m2[i] = pi.nz[i].m2; m3[i] = pi.nz[i].m3; coef[i] = pi.nz[i].c; }
+    return E3_OK;
+}
+
+extern "C" int e3_plan_kernel_info(const e3_plan *plan, int which, int *regs, int *spill_bytes, int *smem_bytes,
+                                   int *threads_per_block, int *n_roles, int *channels_per_lane)
+{
+    if (!plan || (which != 0 && which != 1)) { set_error("e3_plan_kernel_info: bad arguments"); return E3_ERR_INVALID_ARG; }
+    const JitKernel &k = which == 0 ? plan->fwd : plan->bwd;
+    if (regs) *regs = k.regs;
+    if (spill_bytes) *spill_bytes = k.spill;
+    if (smem_bytes) *smem_bytes = k.smem;
+    if (threads_per_block) *threads_per_block = k.threads;
+    if (n_roles) *n_roles = which == 0 ? (int)plan->roles.size() : 1;
+    if (channels_per_lane) *channels_per_lane = plan->K;
+    return E3_OK;
+}
+
+extern "C" int e3_plan_work(const e3_plan *plan, double *fwd_flop_per_edge, double *bwd_flop_per_edge)
+{
+    if (!plan) { set_error("plan is NULL"); return E3_ERR_INVALID_ARG; }
+    double f = 0, b = 0;
+    for (const PathInfo &pi : plan->paths) {
+        f += plan->C * (2.0 * pi.nzM + 2.0 * (2 * pi.l3 + 1)) + 2.0 * pi.nz.size();
+        b += plan->C * (6.0 * pi.nzM + 3.0 * (2 * pi.l3 + 1)) + 4.0 * pi.nz.size();
+    }
+    if (fwd_flop_per_edge) *fwd_flop_per_edge = f;
+    if (bwd_flop_per_edge) *bwd_flop_per_edge = b;
+    return E3_OK;
+}
+
+extern "C" int e3_jit_check(const e3_irrep *irreps_in, int n_in, int sh_lmax, const e3_irrep *irreps_out, int n_out,
+                            const e3_path *paths, int n_paths, e3_dtype dtype, const char *src_path, int *fwd_regs,
+                            int *fwd_spill, int *bwd_regs, int *bwd_spill)
+{
+    e3_plan pl;
+    int rc = plan_build_tables(pl, irreps_in, n_in, sh_lmax, irreps_out, n_out, paths, n_paths, dtype, /*cg_on_device=*/false);
+    if (rc == E3_OK) rc = plan_generate(pl, src_path);
+    if (rc != E3_OK) return rc;
+    if (fwd_regs) *fwd_regs = pl.fwd.regs;
+    if (fwd_spill) *fwd_spill = pl.fwd.spill;
+    if (bwd_regs) *bwd_regs = pl.bwd.regs;
+    if (bwd_spill) *bwd_spill = pl.bwd.spill;
+    return E3_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// graph, SH, forces
+// ---------------------------------------------------------------------------------------------
+extern "C" size_t e3_graph_workspace_bytes(int64_t n_edges, int32_t n_nodes)
+{
+    if (n_edges < 0 || n_nodes < 0) return 0;
+    return graph_workspace_bytes(n_edges, n_nodes);
+}
+
+extern "C" int e3_graph_prepare(const int32_t *senders, const int32_t *receivers, int64_t n_edges, int32_t n_nodes,
+                                int32_t *row_ptr, int32_t *perm_s, int32_t *col_ptr, void *workspace, size_t workspace_bytes,
+                                int validate, e3_stream stream)
+{
+    if (n_edges < 0 || n_nodes < 0 || n_edges > 0x7fffffffLL || !row_ptr || !col_ptr || (n_edges > 0 && (!senders || !receivers || !perm_s))) {
+        set_error("e3_graph_prepare: bad arguments");
+        return E3_ERR_INVALID_ARG;
+    }
+    return launch_graph_prepare(senders, receivers, n_edges, n_nodes, row_ptr, perm_s, col_ptr, workspace, workspace_bytes, validate, S(stream));
+}
+
+extern "C" int e3_sh_fwd(const e3_plan *plan, const float *vec, int64_t n_edges, void *sh, e3_stream stream)
+{
+    if (!plan || n_edges < 0 || (n_edges > 0 && (!vec || !sh))) { set_error("e3_sh_fwd: bad arguments"); return E3_ERR_INVALID_ARG; }
+    return launch_sh_fwd(plan->sh_lmax, plan->dtype, vec, n_edges, sh, S(stream));
+}
+
+extern "C" int e3_sh_bwd(const e3_plan *plan, const float *vec, const float *grad_sh, int64_t n_edges, float *grad_vec, e3_stream stream)
+{
+    if (!plan || n_edges < 0 || (n_edges > 0 && (!vec || !grad_sh || !grad_vec))) { set_error("e3_sh_bwd: bad arguments"); return E3_ERR_INVALID_ARG; }
+    return launch_sh_bwd(plan->sh_lmax, vec, grad_sh, n_edges, grad_vec, S(stream));
+}
+
+extern "C" int e3_force_reduce(const float *grad_vec, const int32_t *row_ptr, const int32_t *perm_s, const int32_t *col_ptr,
+                               int64_t n_edges, int32_t n_nodes, float *forces, e3_stream stream)
+{
+    if (n_edges < 0 || n_nodes < 0 || !row_ptr || !col_ptr || (n_nodes > 0 && !forces) || (n_edges > 0 && (!grad_vec || !perm_s))) {
+        set_error("e3_force_reduce: bad arguments");
+        return E3_ERR_INVALID_ARG;
+    }
+    return launch_force_reduce(grad_vec, row_ptr, perm_s, col_ptr, n_edges, n_nodes, forces, S(stream));
+}
+
+// ---------------------------------------------------------------------------------------------
+// tensor product + scatter
+// ---------------------------------------------------------------------------------------------
+extern "C" int e3_tp_scatter_fwd(const e3_plan *plan, const void *feats, const void *sh, const void *weights,
+                                 const int32_t *senders, const int32_t *receivers, const int32_t *row_ptr, int64_t n_edges,
+                                 int32_t n_nodes, float *out, e3_stream stream)
+{
+    (void)receivers;
+    if (!plan || n_edges < 0 || n_nodes < 0 || !row_ptr || (n_nodes > 0 && (!feats || !out)) ||
+        (n_edges > 0 && (!sh || !weights || !senders))) {
+        set_error("e3_tp_scatter_fwd: bad arguments");
+        return E3_ERR_INVALID_ARG;
+    }
+    if (!aligned16(feats) || !aligned16(weights) || !aligned16(out) || !aligned16(sh)) {
+        set_error("e3_tp_scatter_fwd: tensor pointers must be 16-byte aligned");
+        return E3_ERR_INVALID_ARG;
+    }
+    if (n_nodes == 0) return E3_OK;
+    if (!plan->fwd.fn) { set_error("plan has no loaded forward kernel"); return E3_ERR_CUDA; }
+    long long items = (long long)n_nodes * (long long)plan->roles.size() * plan->nchb;
+    long long grid = (items + plan->fwd_warps - 1) / plan->fwd_warps;
+    if (grid > 0x7fffffffLL) { set_error("grid too large"); return E3_ERR_UNSUPPORTED; }
+    void *args[] = { (void *)&feats, (void *)&sh, (void *)&weights, (void *)&senders, (void *)&row_ptr, (void *)&out, (void *)&n_nodes };
+    E3_CUDA_TRY(cudaLaunchKernel((const void *)plan->fwd.fn, dim3((unsigned)grid), dim3(plan->fwd.threads), args, 0, S(stream)));
+    return E3_OK;
+}
+
+extern "C" size_t e3_bwd_workspace_bytes(const e3_plan *plan, int64_t n_edges, int32_t n_nodes)
+{
+    (void)n_nodes;
+    if (!plan || n_edges < 0) return 0;
+    return (size_t)n_edges * plan->in_dim * plan->C * sizeof(float) + 256;
+}
+
+extern "C" int e3_tp_scatter_bwd(const e3_plan *plan, const void *feats, const void *sh, const void *weights,
+                                 const int32_t *senders, const int32_t *receivers, const int32_t *row_ptr, const int32_t *perm_s,
+                                 const int32_t *col_ptr, int64_t n_edges, int32_t n_nodes, const float *grad_out,
+                                 float *grad_feats, float *grad_sh, void *grad_weights, void *workspace, size_t workspace_bytes,
+                                 e3_stream stream)
+{
+    (void)row_ptr;
+    if (!plan || n_edges < 0 || n_nodes < 0 || !col_ptr || (n_nodes > 0 && (!feats || !grad_out || !grad_feats)) ||
+        (n_edges > 0 && (!sh || !weights || !senders || !receivers || !perm_s || !grad_sh))) {
+        set_error("e3_tp_scatter_bwd: bad arguments");
+        return E3_ERR_INVALID_ARG;
+    }
+    if (!aligned16(feats) || !aligned16(weights) || !aligned16(grad_out) || !aligned16(grad_feats) || !aligned16(grad_weights) ||
+        !aligned16(sh) || !aligned16(workspace)) {
+        set_error("e3_tp_scatter_bwd: tensor pointers must be 16-byte aligned");
+        return E3_ERR_INVALID_ARG;
+    }
+    if (n_edges > 0 && (!workspace || workspace_bytes < e3_bwd_workspace_bytes(plan, n_edges, n_nodes))) {
+        set_error("e3_tp_scatter_bwd: workspace too small (need %zu bytes)", e3_bwd_workspace_bytes(plan, n_edges, n_nodes));
+        return E3_ERR_WORKSPACE;
+    }
+    if (n_nodes == 0) return E3_OK;
+    if (!plan->bwd.fn) { set_error("plan has no loaded backward kernel"); return E3_ERR_CUDA; }
+    float *dxe = (float *)workspace;
+    if (n_edges > 0) {
+        long long warps = (n_edges + plan->bwd_edges_per_warp - 1) / plan->bwd_edges_per_warp;
+        long long grid = (warps + plan->bwd_warps - 1) / plan->bwd_warps;
+        long long ne = n_edges;
+        void *args[] = { (void *)&feats, (void *)&sh, (void *)&weights, (void *)&senders, (void *)&receivers, (void *)&grad_out,
+                         (void *)&dxe, (void *)&grad_sh, (void *)&grad_weights, (void *)&ne };
+        E3_CUDA_TRY(cudaLaunchKernel((const void *)plan->bwd.fn, dim3((unsigned)grid), dim3(plan->bwd.threads), args, 0, S(stream)));
+    }
+    return launch_dx_reduce(dxe, perm_s, col_ptr, n_nodes, plan->in_dim * plan->C, grad_feats, S(stream));
+}
+
+// ---------------------------------------------------------------------------------------------
+// host-buffer session
+// ---------------------------------------------------------------------------------------------
+struct e3_session {
+    const e3_plan *plan = nullptr;
+    int64_t max_edges = 0;
+    int32_t max_nodes = 0;
+    cudaStream_t stream = nullptr;
+    float *vec = nullptr, *out = nullptr, *gout = nullptr, *gfeats = nullptr, *gsh = nullptr, *gvec = nullptr, *forces = nullptr;
+    void *feats = nullptr, *sh = nullptr, *weights = nullptr, *gweights = nullptr, *ws = nullptr, *gws = nullptr;
+    int32_t *snd = nullptr, *rcv = nullptr, *row_ptr = nullptr, *perm_s = nullptr, *col_ptr = nullptr;
+    size_t ws_bytes = 0, gws_bytes = 0;
+};
+
+extern "C" int e3_session_destroy(e3_session *s)
+{
+    if (!s) return E3_OK;
+    void *ptrs[] = { s->vec, s->out, s->gout, s->gfeats, s->gsh, s->gvec, s->forces, s->feats, s->sh, s->weights, s->gweights,
+                     s->ws, s->gws, s->snd, s->rcv, s->row_ptr, s->perm_s, s->col_ptr };
+    for (void *p : ptrs) if (p) cudaFree(p);
+    if (s->stream) cudaStreamDestroy(s->stream);
+    delete s;
+    return E3_OK;
+}
+
+extern "C" int e3_session_create(e3_session **session, const e3_plan *plan, int64_t max_edges, int32_t max_nodes)
+{
+    if (!session || !plan || max_edges < 0 || max_nodes < 0) { set_error("e3_session_create: bad arguments"); return E3_ERR_INVALID_ARG; }
+    *session = nullptr;
+    e3_session *s = new (std::nothrow) e3_session();
+    if (!s) { set_error("out of host memory"); return E3_ERR_INVALID_ARG; }
+    s->plan = plan; s->max_edges = max_edges; s->max_nodes = max_nodes;
+    const size_t E = (size_t)max_edges + 1, N = (size_t)max_nodes + 1, es = esize(plan);
+    const size_t P = plan->paths.size(), C = plan->C;
+    s->ws_bytes = e3_bwd_workspace_bytes(plan, max_edges, max_nodes);
+    s->gws_bytes = graph_workspace_bytes(max_edges, max_nodes);
+    cudaError_t e = cudaStreamCreateWithFlags(&s->stream, cudaStreamNonBlocking);
+#define SALLOC(ptr, bytes) if (e == cudaSuccess) e = cudaMalloc((void **)&(ptr), (bytes))
+    SALLOC(s->vec, E * 3 * 4); SALLOC(s->gvec, E * 3 * 4); SALLOC(s->forces, N * 3 * 4);
+    SALLOC(s->feats, N * plan->in_dim * C * es); SALLOC(s->gfeats, N * plan->in_dim * C * 4);
+    SALLOC(s->out, N * plan->out_dim * C * 4); SALLOC(s->gout, N * plan->out_dim * C * 4);
+    SALLOC(s->sh, E * plan->sh_dim * es); SALLOC(s->gsh, E * plan->sh_dim * 4);
+    SALLOC(s->weights, E * P * C * es); SALLOC(s->gweights, E * P * C * es);
+    SALLOC(s->ws, s->ws_bytes); SALLOC(s->gws, s->gws_bytes);
+    SALLOC(s->snd, E * 4); SALLOC(s->rcv, E * 4); SALLOC(s->row_ptr, (N + 1) * 4); SALLOC(s->perm_s, E * 4); SALLOC(s->col_ptr, (N + 1) * 4);
+#undef SALLOC
+    if (e != cudaSuccess) { e3_session_destroy(s); return cuda_fail(e, "session allocation"); }
+    *session = s;
+    return E3_OK;
+}
+
+extern "C" int e3_session_run_host(e3_session *s, const float *vec_h, const void *feats_h, const void *weights_h,
+                                   const int32_t *senders_h, const int32_t *receivers_h, int64_t n_edges, int32_t n_nodes,
+                                   const float *grad_out_h, float *out_h, float *grad_feats_h, void *grad_weights_h,
+                                   float *grad_vec_h, float *forces_h, int64_t *bytes_h2d, int64_t *bytes_d2h)
+{
+    if (!s || n_edges < 0 || n_nodes < 0 || n_edges > s->max_edges || n_nodes > s->max_nodes ||
+        (n_nodes > 0 && !feats_h) || (n_edges > 0 && (!vec_h || !weights_h || !senders_h || !receivers_h))) {
+        set_error("e3_session_run_host: bad arguments or sizes above the session capacity");
+        return E3_ERR_INVALID_ARG;
+    }
+    const e3_plan *pl = s->plan;
+    const size_t E = (size_t)n_edges, N = (size_t)n_nodes, es = esize(pl), P = pl->paths.size(), C = pl->C;
+    cudaStream_t st = s->stream;
+    int64_t up = 0, down = 0;
+#define H2D(dst, src, bytes) do { if ((bytes) > 0) { E3_CUDA_TRY(cudaMemcpyAsync((dst), (src), (bytes), cudaMemcpyHostToDevice, st)); up += (int64_t)(bytes); } } while (0)
+#define D2H(dst, src, bytes) do { if ((dst) && (bytes) > 0) { E3_CUDA_TRY(cudaMemcpyAsync((dst), (src), (bytes), cudaMemcpyDeviceToHost, st)); down += (int64_t)(bytes); } } while (0)
+    H2D(s->snd, senders_h, E * 4); H2D(s->rcv, receivers_h, E * 4); H2D(s->vec, vec_h, E * 12);
+    H2D(s->feats, feats_h, N * pl->in_dim * C * es); H2D(s->weights, weights_h, E * P * C * es);
+    int rc = launch_graph_prepare(s->snd, s->rcv, n_edges, n_nodes, s->row_ptr, s->perm_s, s->col_ptr, s->gws, s->gws_bytes, 0, st);
+    if (rc == E3_OK) rc = e3_sh_fwd(pl, s->vec, n_edges, s->sh, st);
+    if (rc == E3_OK) rc = e3_tp_scatter_fwd(pl, s->feats, s->sh, s->weights, s->snd, s->rcv, s->row_ptr, n_edges, n_nodes, s->out, st);
+    if (rc != E3_OK) return rc;
+    D2H(out_h, s->out, N * pl->out_dim * C * 4);
+    if (grad_out_h) {
+        H2D(s->gout, grad_out_h, N * pl->out_dim * C * 4);
+        rc = e3_tp_scatter_bwd(pl, s->feats, s->sh, s->weights, s->snd, s->rcv, s->row_ptr, s->perm_s, s->col_ptr, n_edges, n_nodes,
+                               s->gout, s->gfeats, s->gsh, grad_weights_h ? s->gweights : nullptr, s->ws, s->ws_bytes, st);
+        if (rc == E3_OK) rc = e3_sh_bwd(pl, s->vec, s->gsh, n_edges, s->gvec, st);
+        if (rc == E3_OK && forces_h) rc = e3_force_reduce(s->gvec, s->row_ptr, s->perm_s, s->col_ptr, n_edges, n_nodes, s->forces, st);
+        if (rc != E3_OK) return rc;
+        D2H(grad_feats_h, s->gfeats, N * pl->in_dim * C * 4);
+        D2H(grad_weights_h, s->gweights, E * P * C * es);
+        D2H(grad_vec_h, s->gvec, E * 12);
+        D2H(forces_h, s->forces, N * 12);
+    }
+#undef H2D
+#undef D2H
+    E3_CUDA_TRY(cudaStreamSynchronize(st));
+    if (bytes_h2d) *bytes_h2d = up;
+    if (bytes_d2h) *bytes_d2h = down;
+    return E3_OK;
+}

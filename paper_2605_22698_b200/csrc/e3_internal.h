@@ -1,0 +1,101 @@
+// Internal declarations shared by the translation units of libe3b200.so (never installed).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdarg>
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/e3b200.h"
+
+namespace e3 {
+
+constexpr int kMaxL = 3;      // highest degree supported anywhere (irreps, SH)
+constexpr int kMaxShDim = 16;
+
+// thread-local error detail -------------------------------------------------------------------
+void set_error(const char *fmt, ...);
+const char *get_error();
+int cuda_fail(cudaError_t e, const char *what);     // records text, returns E3_ERR_CUDA
+
+#define E3_CUDA_TRY(expr)                                          \
+    do {                                                           \
+        cudaError_t e3_err__ = (expr);                             \
+        if (e3_err__ != cudaSuccess) return ::e3::cuda_fail(e3_err__, #expr); \
+    } while (0)
+
+// one non-zero of a real Clebsch-Gordan tensor (indices 0-based: m_true + l)
+struct Nz { int m1, m2, m3; double c; };
+
+struct PathInfo {
+    int i_in, l_sh, i_out;     // as given by the caller
+    int l1, l2, l3;
+    int in_off, out_off;       // first row (in units of C-wide rows) of the irrep block in a node row
+    std::vector<Nz> nz;        // sparse real CG, ordered m1, m2, m3
+    int nzM;                   // structurally non-zero (m1, m3) pairs
+};
+
+// A forward "role": a set of output irreps (and every path feeding them) owned by one warp.
+struct Role {
+    std::vector<int> out_irreps;
+    std::vector<int> paths;
+    int rows;                  // accumulator rows (sum of 2l3+1 over out_irreps)
+    double cost;
+};
+
+struct JitKernel {
+    std::string name;
+    std::string source;
+    std::vector<char> cubin;
+    int regs = 0, spill = 0, smem = 0, threads = 0;
+    cudaLibrary_t lib = nullptr;
+    cudaKernel_t fn = nullptr;
+};
+
+}  // namespace e3
+
+struct e3_plan {
+    std::vector<e3_irrep> irreps_in, irreps_out;
+    std::vector<e3::PathInfo> paths;
+    int sh_lmax = 0, sh_dim = 0, in_dim = 0, out_dim = 0, C = 0;
+    e3_dtype dtype = E3_F32;
+    int nnz_total = 0;
+    // launch geometry chosen by the code generator
+    int K = 1;                 // channels per lane
+    int nchb = 1;              // channel blocks of 32*K
+    std::vector<e3::Role> roles;
+    int fwd_warps = 4, bwd_warps = 4, bwd_edges_per_warp = 8;
+    e3::JitKernel fwd, bwd;
+};
+
+namespace e3 {
+
+// plan.cu
+double cg_real_host(int l1, int l2, int l3, int m1, int m2, int m3);   // same routine as the device planner kernel
+int plan_build_tables(e3_plan &pl, const e3_irrep *irreps_in, int n_in, int sh_lmax, const e3_irrep *irreps_out,
+                      int n_out, const e3_path *paths, int n_paths, e3_dtype dtype, bool cg_on_device);
+void plan_make_roles(e3_plan &pl);
+
+// codegen.cpp
+std::string gen_forward_source(const e3_plan &pl);
+std::string gen_backward_source(const e3_plan &pl);
+
+// jit.cpp
+int jit_compile(JitKernel &k, const std::string &file_hint);   // NVRTC -> cubin (+regs/spill from the ptxas log)
+int jit_load(JitKernel &k);                                    // cubin -> cudaKernel_t (needs a device)
+void jit_unload(JitKernel &k);
+
+// kernels.cu (statically compiled kernels)
+int launch_sh_fwd(int lmax, e3_dtype dt, const float *vec, int64_t E, void *sh, cudaStream_t st);
+int launch_sh_bwd(int lmax, const float *vec, const float *gsh, int64_t E, float *gvec, cudaStream_t st);
+size_t graph_workspace_bytes(int64_t E, int32_t N);
+int launch_graph_prepare(const int32_t *snd, const int32_t *rcv, int64_t E, int32_t N, int32_t *row_ptr,
+                         int32_t *perm_s, int32_t *col_ptr, void *ws, size_t ws_bytes, int validate, cudaStream_t st);
+int launch_force_reduce(const float *gvec, const int32_t *row_ptr, const int32_t *perm_s, const int32_t *col_ptr,
+                        int64_t E, int32_t N, float *forces, cudaStream_t st);
+int launch_dx_reduce(const float *dxe, const int32_t *perm_s, const int32_t *col_ptr, int32_t N, int row_len,
+                     float *dx, cudaStream_t st);
+int launch_cg_planner(const int *triples /*[n,3] host*/, int n, std::vector<std::vector<double>> &dense_out);
+
+}  // namespace e3

@@ -1,0 +1,354 @@
+// Statically compiled kernels: spherical harmonics fwd/bwd (a2, a6), graph preparation (a3),
+// force reduction (a7) and the per-sender reduction that finishes grad_feats (second phase of a5).
+#include <cuda_bf16.h>
+
+#include "e3_internal.h"
+
+namespace e3 {
+
+// ---------------------------------------------------------------------------------------------
+// Real spherical harmonics, component normalisation, l <= 3 (readings A1-A3).
+// x,y,z is the unit vector; written as explicit polynomials.
+// ---------------------------------------------------------------------------------------------
+#define SQ3 1.7320508075688772f
+#define SQ5 2.2360679774997897f
+#define SQ7 2.6457513110645906f
+#define SQ15 3.8729833462074170f
+#define SQ42 6.4807406984078604f
+#define SQ70 8.3666002653407556f
+#define SQ105 10.246950765959598f
+
+template <int LMAX>
+__device__ __forceinline__ void sh_values(float x, float y, float z, float nz, float *Y)
+{
+    // nz = 1 for a regular vector, 0 for the zero vector (A3: Y_00 = 1, everything else 0)
+    Y[0] = 1.0f;
+    if (LMAX >= 1) { Y[1] = SQ3 * y; Y[2] = SQ3 * z; Y[3] = SQ3 * x; }
+    if (LMAX >= 2) {
+        Y[4] = SQ15 * x * y;
+        Y[5] = SQ15 * y * z;
+        Y[6] = (0.5f * SQ5) * (3.0f * z * z - nz);
+        Y[7] = SQ15 * x * z;
+        Y[8] = (0.5f * SQ15) * (x * x - y * y);
+    }
+    if (LMAX >= 3) {
+        float x2 = x * x, y2 = y * y, z2 = z * z;
+        Y[9] = (0.25f * SQ70) * y * (3.0f * x2 - y2);
+        Y[10] = SQ105 * x * y * z;
+        Y[11] = (0.25f * SQ42) * y * (5.0f * z2 - nz);
+        Y[12] = (0.5f * SQ7) * z * (5.0f * z2 - 3.0f * nz);
+        Y[13] = (0.25f * SQ42) * x * (5.0f * z2 - nz);
+        Y[14] = (0.5f * SQ105) * z * (x2 - y2);
+        Y[15] = (0.25f * SQ70) * x * (x2 - 3.0f * y2);
+    }
+}
+
+template <int LMAX, typename T>
+__global__ void __launch_bounds__(128) sh_fwd_kernel(const float *__restrict__ vec, int64_t E, T *__restrict__ sh)
+{
+    constexpr int D = (LMAX + 1) * (LMAX + 1);
+    constexpr int DP = D | 1;                         // odd stride: conflict-free staging
+    __shared__ float stage[128 * DP];
+    const int64_t base = (int64_t)blockIdx.x * 128;
+    const int64_t e = base + threadIdx.x;
+    if (e < E) {
+        float vx = vec[3 * e], vy = vec[3 * e + 1], vz = vec[3 * e + 2];
+        float n2 = vx * vx + vy * vy + vz * vz;
+        float inv = n2 > 0.0f ? 1.0f / sqrtf(n2) : 0.0f;
+        float Y[D];
+        sh_values<LMAX>(vx * inv, vy * inv, vz * inv, n2 > 0.0f ? 1.0f : 0.0f, Y);
+#pragma unroll
+        for (int i = 0; i < D; ++i) stage[threadIdx.x * DP + i] = Y[i];
+    }
+    __syncthreads();
+    const int64_t n_here = (E - base < 128 ? E - base : 128) * D;
+    for (int64_t j = threadIdx.x; j < n_here; j += 128) {
+        int le = (int)(j / D), c = (int)(j % D);
+        float v = stage[le * DP + c];
+        if constexpr (sizeof(T) == 2) sh[base * D + j] = __float2bfloat16_rn(v);
+        else sh[base * D + j] = v;
+    }
+}
+
+// grad_vec = (1/|r|) (I - r^ r^T) sum_lm grad_sh[lm] * grad F_lm(r^)
+template <int LMAX>
+__global__ void __launch_bounds__(128) sh_bwd_kernel(const float *__restrict__ vec, const float *__restrict__ gsh,
+                                                     int64_t E, float *__restrict__ gvec)
+{
+    constexpr int D = (LMAX + 1) * (LMAX + 1);
+    const int64_t e = (int64_t)blockIdx.x * 128 + threadIdx.x;
+    if (e >= E) return;
+    float vx = vec[3 * e], vy = vec[3 * e + 1], vz = vec[3 * e + 2];
+    float n2 = vx * vx + vy * vy + vz * vz;
+    if (!(n2 > 0.0f)) { gvec[3 * e] = 0.0f; gvec[3 * e + 1] = 0.0f; gvec[3 * e + 2] = 0.0f; return; }
+    float inv = 1.0f / sqrtf(n2);
+    float x = vx * inv, y = vy * inv, z = vz * inv;
+    float g[D];
+#pragma unroll
+    for (int i = 0; i < D; ++i) g[i] = gsh[e * D + i];
+    float gx = 0.0f, gy = 0.0f, gz = 0.0f;
+    if (LMAX >= 1) { gy += SQ3 * g[1]; gz += SQ3 * g[2]; gx += SQ3 * g[3]; }
+    if (LMAX >= 2) {
+        gx += SQ15 * (g[4] * y + g[7] * z + g[8] * x);
+        gy += SQ15 * (g[4] * x + g[5] * z - g[8] * y);
+        gz += SQ15 * (g[5] * y + g[7] * x) + (3.0f * SQ5) * g[6] * z;
+    }
+    if (LMAX >= 3) {
+        float x2 = x * x, y2 = y * y, z2 = z * z;
+        float a = 0.25f * SQ70, b = SQ105, c = 0.25f * SQ42, d = 0.5f * SQ7, f = 0.5f * SQ105;
+        gx += a * g[9] * (6.0f * x * y) + b * g[10] * (y * z) + c * g[13] * (5.0f * z2 - 1.0f)
+              + f * g[14] * (2.0f * x * z) + a * g[15] * (3.0f * x2 - 3.0f * y2);
+        gy += a * g[9] * (3.0f * x2 - 3.0f * y2) + b * g[10] * (x * z) + c * g[11] * (5.0f * z2 - 1.0f)
+              - f * g[14] * (2.0f * y * z) - a * g[15] * (6.0f * x * y);
+        gz += b * g[10] * (x * y) + c * g[11] * (10.0f * y * z) + d * g[12] * (15.0f * z2 - 3.0f)
+              + c * g[13] * (10.0f * x * z) + f * g[14] * (x2 - y2);
+    }
+    float rad = gx * x + gy * y + gz * z;
+    gvec[3 * e] = (gx - x * rad) * inv;
+    gvec[3 * e + 1] = (gy - y * rad) * inv;
+    gvec[3 * e + 2] = (gz - z * rad) * inv;
+}
+
+int launch_sh_fwd(int lmax, e3_dtype dt, const float *vec, int64_t E, void *sh, cudaStream_t st)
+{
+    if (E == 0) return E3_OK;
+    unsigned grid = (unsigned)((E + 127) / 128);
+#define SH_CASE(L)                                                                                          \
+    case L:                                                                                                 \
+        if (dt == E3_BF16) sh_fwd_kernel<L, __nv_bfloat16><<<grid, 128, 0, st>>>(vec, E, (__nv_bfloat16 *)sh); \
+        else sh_fwd_kernel<L, float><<<grid, 128, 0, st>>>(vec, E, (float *)sh);                            \
+        break;
+    switch (lmax) { SH_CASE(0) SH_CASE(1) SH_CASE(2) SH_CASE(3) default: set_error("sh: lmax %d unsupported", lmax); return E3_ERR_UNSUPPORTED; }
+#undef SH_CASE
+    E3_CUDA_TRY(cudaGetLastError());
+    return E3_OK;
+}
+
+int launch_sh_bwd(int lmax, const float *vec, const float *gsh, int64_t E, float *gvec, cudaStream_t st)
+{
+    if (E == 0) return E3_OK;
+    unsigned grid = (unsigned)((E + 127) / 128);
+    switch (lmax) {
+    case 0: sh_bwd_kernel<0><<<grid, 128, 0, st>>>(vec, gsh, E, gvec); break;
+    case 1: sh_bwd_kernel<1><<<grid, 128, 0, st>>>(vec, gsh, E, gvec); break;
+    case 2: sh_bwd_kernel<2><<<grid, 128, 0, st>>>(vec, gsh, E, gvec); break;
+    case 3: sh_bwd_kernel<3><<<grid, 128, 0, st>>>(vec, gsh, E, gvec); break;
+    default: set_error("sh: lmax %d unsupported", lmax); return E3_ERR_UNSUPPORTED;
+    }
+    E3_CUDA_TRY(cudaGetLastError());
+    return E3_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Graph preparation: integer only, result unique (A15).
+// workspace ints: [0] flags, [4 .. 4+N) cursor, [4+N .. 4+N+E) unsorted fill
+// ---------------------------------------------------------------------------------------------
+size_t graph_workspace_bytes(int64_t E, int32_t N) { return sizeof(int32_t) * (size_t)(4 + (int64_t)N + E + 4); }
+
+__global__ void graph_validate_kernel(const int32_t *__restrict__ snd, const int32_t *__restrict__ rcv, int64_t E,
+                                      int32_t N, int32_t *flags)
+{
+    int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= E) return;
+    int f = 0;
+    if (snd[e] < 0 || snd[e] >= N || rcv[e] < 0 || rcv[e] >= N) f |= 1;
+    if (e > 0 && rcv[e] < rcv[e - 1]) f |= 2;
+    if (f) atomicOr(flags, f);
+}
+
+// row_ptr from receiver-sorted edges: thread e (0..E) fills the pointer entries that fall between
+// receivers[e-1] and receivers[e]
+__global__ void graph_row_ptr_kernel(const int32_t *__restrict__ rcv, int64_t E, int32_t N, int32_t *__restrict__ row_ptr)
+{
+    int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e > E) return;
+    int32_t lo = (e == 0) ? 0 : rcv[e - 1] + 1;
+    int32_t hi = (e == E) ? N : rcv[e];
+    for (int32_t r = lo; r <= hi; ++r) row_ptr[r] = (int32_t)e;
+}
+
+__global__ void graph_count_kernel(const int32_t *__restrict__ snd, int64_t E, int32_t *__restrict__ col_ptr)
+{
+    int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e < E) atomicAdd(&col_ptr[snd[e] + 1], 1);     // integer atomics: order-independent result
+}
+
+// in-place inclusive scan of col_ptr[0..N] by one block (N+1 entries), then cursor = col_ptr[0..N)
+__global__ void __launch_bounds__(1024) graph_scan_kernel(int32_t *__restrict__ col_ptr, int32_t n, int32_t *__restrict__ cursor)
+{
+    __shared__ int32_t warp_sum[32];
+    __shared__ int32_t carry_s;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    for (int32_t base = 0; base < n; base += 1024) {
+        int32_t i = base + threadIdx.x;
+        int32_t v = (i < n) ? col_ptr[i] : 0;
+        int32_t s = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { int32_t t = __shfl_up_sync(0xffffffffu, s, o); if (lane >= o) s += t; }
+        if (lane == 31) warp_sum[wid] = s;
+        __syncthreads();
+        if (wid == 0) {
+            int32_t w = warp_sum[lane];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { int32_t t = __shfl_up_sync(0xffffffffu, w, o); if (lane >= o) w += t; }
+            warp_sum[lane] = w;
+        }
+        __syncthreads();
+        int32_t carry = carry_s;
+        int32_t incl = s + (wid > 0 ? warp_sum[wid - 1] : 0) + carry;
+        if (i < n) { col_ptr[i] = incl; if (i < n - 1) cursor[i] = incl; }
+        __syncthreads();
+        if (threadIdx.x == 1023) carry_s = incl;
+        __syncthreads();
+    }
+}
+
+__global__ void graph_fill_kernel(const int32_t *__restrict__ snd, int64_t E, int32_t *__restrict__ cursor,
+                                  int32_t *__restrict__ fill)
+{
+    int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e < E) fill[atomicAdd(&cursor[snd[e]], 1)] = (int32_t)e;
+}
+
+// one warp per sender: rank-sort its (arbitrarily ordered) segment of edge ids ascending
+__global__ void graph_segment_sort_kernel(const int32_t *__restrict__ col_ptr, const int32_t *__restrict__ fill,
+                                          int32_t N, int32_t *__restrict__ perm_s)
+{
+    int32_t s = (int32_t)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
+    if (s >= N) return;
+    const int lane = threadIdx.x & 31;
+    const int32_t a = col_ptr[s], b = col_ptr[s + 1];
+    for (int32_t i = a + lane; i < b; i += 32) {
+        int32_t v = fill[i];
+        int32_t rank = 0;
+        for (int32_t j = a; j < b; ++j) rank += (fill[j] < v);
+        perm_s[a + rank] = v;
+    }
+}
+
+int launch_graph_prepare(const int32_t *snd, const int32_t *rcv, int64_t E, int32_t N, int32_t *row_ptr,
+                         int32_t *perm_s, int32_t *col_ptr, void *ws, size_t ws_bytes, int validate, cudaStream_t st)
+{
+    if (ws_bytes < graph_workspace_bytes(E, N) || !ws) { set_error("graph_prepare: workspace too small"); return E3_ERR_WORKSPACE; }
+    int32_t *flags = (int32_t *)ws;
+    int32_t *cursor = flags + 4;
+    int32_t *fill = cursor + N;
+    const unsigned tb = 256;
+    const unsigned ge = (unsigned)((E + tb - 1) / tb);
+    if (validate) {
+        E3_CUDA_TRY(cudaMemsetAsync(flags, 0, sizeof(int32_t) * 4, st));
+        if (E > 0) graph_validate_kernel<<<ge, tb, 0, st>>>(snd, rcv, E, N, flags);
+        int32_t h = 0;
+        E3_CUDA_TRY(cudaMemcpyAsync(&h, flags, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+        E3_CUDA_TRY(cudaStreamSynchronize(st));
+        if (h & 1) { set_error("graph_prepare: sender/receiver index out of range"); return E3_ERR_INVALID_ARG; }
+        if (h & 2) { set_error("graph_prepare: receivers are not sorted ascending"); return E3_ERR_UNSORTED; }
+    }
+    graph_row_ptr_kernel<<<(unsigned)((E + 1 + tb - 1) / tb), tb, 0, st>>>(rcv, E, N, row_ptr);
+    E3_CUDA_TRY(cudaMemsetAsync(col_ptr, 0, sizeof(int32_t) * ((size_t)N + 1), st));
+    if (E > 0) graph_count_kernel<<<ge, tb, 0, st>>>(snd, E, col_ptr);
+    graph_scan_kernel<<<1, 1024, 0, st>>>(col_ptr, N + 1, cursor);
+    if (E > 0) {
+        graph_fill_kernel<<<ge, tb, 0, st>>>(snd, E, cursor, fill);
+        graph_segment_sort_kernel<<<(unsigned)(((int64_t)N * 32 + tb - 1) / tb), tb, 0, st>>>(col_ptr, fill, N, perm_s);
+    }
+    E3_CUDA_TRY(cudaGetLastError());
+    return E3_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// forces[i] = -( sum_{in-edges} gvec - sum_{out-edges} gvec ), one warp per atom, fixed order
+// ---------------------------------------------------------------------------------------------
+__global__ void force_reduce_kernel(const float *__restrict__ gvec, const int32_t *__restrict__ row_ptr,
+                                    const int32_t *__restrict__ perm_s, const int32_t *__restrict__ col_ptr,
+                                    int32_t N, float *__restrict__ forces)
+{
+    int32_t i = (int32_t)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
+    if (i >= N) return;
+    const int lane = threadIdx.x & 31;
+    float fx = 0.0f, fy = 0.0f, fz = 0.0f;
+    for (int32_t e = row_ptr[i] + lane; e < row_ptr[i + 1]; e += 32) {
+        fx -= gvec[3 * (int64_t)e]; fy -= gvec[3 * (int64_t)e + 1]; fz -= gvec[3 * (int64_t)e + 2];
+    }
+    for (int32_t j = col_ptr[i] + lane; j < col_ptr[i + 1]; j += 32) {
+        int64_t e = perm_s[j];
+        fx += gvec[3 * e]; fy += gvec[3 * e + 1]; fz += gvec[3 * e + 2];
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        fx += __shfl_xor_sync(0xffffffffu, fx, o);
+        fy += __shfl_xor_sync(0xffffffffu, fy, o);
+        fz += __shfl_xor_sync(0xffffffffu, fz, o);
+    }
+    if (lane == 0) { forces[3 * (int64_t)i] = fx; forces[3 * (int64_t)i + 1] = fy; forces[3 * (int64_t)i + 2] = fz; }
+}
+
+int launch_force_reduce(const float *gvec, const int32_t *row_ptr, const int32_t *perm_s, const int32_t *col_ptr,
+                        int64_t E, int32_t N, float *forces, cudaStream_t st)
+{
+    (void)E;
+    if (N == 0) return E3_OK;
+    const unsigned tb = 256;
+    force_reduce_kernel<<<(unsigned)(((int64_t)N * 32 + tb - 1) / tb), tb, 0, st>>>(gvec, row_ptr, perm_s, col_ptr, N, forces);
+    E3_CUDA_TRY(cudaGetLastError());
+    return E3_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// grad_feats[s, :] = sum over the out-edges of s (ascending edge id) of the per-edge rows written
+// by the first VJP phase.  grid.x = sender, threads over columns; VEC floats per thread.
+// ---------------------------------------------------------------------------------------------
+template <int VEC>
+__global__ void dx_reduce_kernel(const float *__restrict__ dxe, const int32_t *__restrict__ perm_s,
+                                 const int32_t *__restrict__ col_ptr, int row_len, float *__restrict__ dx)
+{
+    const int32_t s = blockIdx.x;
+    const int32_t a = col_ptr[s], b = col_ptr[s + 1];
+    for (int c = threadIdx.x * VEC; c < row_len; c += blockDim.x * VEC) {
+        float acc[VEC];
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) acc[v] = 0.0f;
+        int32_t j = a;
+        for (; j + 4 <= b; j += 4) {
+            float t[4][VEC];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const float *row = dxe + (size_t)perm_s[j + q] * row_len + c;
+                if constexpr (VEC == 4) { float4 v4 = *reinterpret_cast<const float4 *>(row); t[q][0] = v4.x; t[q][1] = v4.y; t[q][2] = v4.z; t[q][3] = v4.w; }
+                else t[q][0] = row[0];
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+#pragma unroll
+                for (int v = 0; v < VEC; ++v) acc[v] += t[q][v];
+        }
+        for (; j < b; ++j) {
+            const float *row = dxe + (size_t)perm_s[j] * row_len + c;
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) acc[v] += row[v];
+        }
+        float *o = dx + (size_t)s * row_len + c;
+        if constexpr (VEC == 4) *reinterpret_cast<float4 *>(o) = make_float4(acc[0], acc[1], acc[2], acc[3]);
+        else o[0] = acc[0];
+    }
+}
+
+int launch_dx_reduce(const float *dxe, const int32_t *perm_s, const int32_t *col_ptr, int32_t N, int row_len,
+                     float *dx, cudaStream_t st)
+{
+    if (N == 0) return E3_OK;
+    if (row_len % 4 == 0) {
+        int th = row_len / 4;
+        th = th > 256 ? 256 : ((th + 31) / 32) * 32;
+        dx_reduce_kernel<4><<<(unsigned)N, th, 0, st>>>(dxe, perm_s, col_ptr, row_len, dx);
+    } else {
+        int th = row_len > 256 ? 256 : ((row_len + 31) / 32) * 32;
+        dx_reduce_kernel<1><<<(unsigned)N, th, 0, st>>>(dxe, perm_s, col_ptr, row_len, dx);
+    }
+    E3_CUDA_TRY(cudaGetLastError());
+    return E3_OK;
+}
+
+}  // namespace e3

@@ -33,3 +33,12 @@ def read_golden(name):
             if line:
                 rows.append(line.split())
     return rows
+
+
+def pytest_sessionstart(session):
+    """Make sure both shared libraries exist (cheap when up to date): the gcc-built oracle and the
+    nvcc-built CUDA library.  Building is not using: no test computes through a missing library."""
+    import oracle
+    from paper_2605_22698_b200 import build as lib_build
+    oracle.build()
+    lib_build.build()

@@ -1,0 +1,81 @@
+"""CPU-side checks of the CUDA library: it loads, exports every symbol the header declares, its host
+logic (path enumeration, validation) is right, the plan kernels compile for sm_100a, and compute
+calls fail loudly without a device (there is no CPU fallback)."""
+import ctypes
+import os
+import re
+
+import pytest
+import torch
+
+import oracle as O
+from paper_2605_22698_b200 import binding as B
+from paper_2605_22698_b200 import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_loads_and_exports_every_declared_symbol():
+    L = B.lib()
+    header = open(os.path.join(ROOT, "include", "e3b200.h")).read()
+    declared = set(re.findall(r"\b(e3_[a-z_0-9]+)\s*\(", header))
+    declared -= {"e3_plan", "e3_session"}
+    assert declared == set(B.SYMBOLS), declared ^ set(B.SYMBOLS)
+    for name in declared:
+        assert hasattr(L, name), name
+    assert L.e3_status_string(0) == b"ok"
+    assert b"sorted" in L.e3_status_string(B.E3_ERR_UNSORTED)
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
+@pytest.mark.parametrize("natural", [False, True])
+def test_all_paths_matches_oracle_enumerator(k, natural):
+    cfg = W.CONFIGS[k]
+    ii = [(l, p, cfg.channels) for l, p in cfg.irreps_in]
+    io, pp = B.e3_all_paths(ii, cfg.sh_lmax, cfg.out_lmax, natural)
+    io_ref, pp_ref = O.all_paths(ii, cfg.sh_lmax, cfg.out_lmax, natural)
+    assert io == [tuple(t) for t in io_ref] and pp == [tuple(t) for t in pp_ref]
+    expect = {1: (15, 11), 2: (13, 10), 3: (15, 11), 4: (34, 23), 5: (34, 23)}[k]
+    assert len(pp) == expect[1 if natural else 0]
+
+
+def test_jit_check_compiles_without_spills_small_plans():
+    for k in (1, 2, 3):
+        cfg = W.CONFIGS[k]
+        ii = [(l, p, cfg.channels) for l, p in cfg.irreps_in]
+        io, pp = B.e3_all_paths(ii, cfg.sh_lmax, cfg.out_lmax)
+        r = B.e3_jit_check(ii, cfg.sh_lmax, io, pp, B.E3_F32)
+        assert r["fwd_regs"] > 0 and r["bwd_regs"] > 0 and r["fwd_spill"] == 0 and r["bwd_spill"] == 0, r
+
+
+def test_jit_check_rejects_bad_plans():
+    C = 4
+    with pytest.raises(B.E3Error) as e:        # triangle
+        B.e3_jit_check([(0, 1, C)], 1, [(0, 1, C)], [(0, 1, 0)])
+    assert e.value.status == B.E3_ERR_BAD_PATH
+    with pytest.raises(B.E3Error) as e:        # parity
+        B.e3_jit_check([(0, 1, C)], 1, [(1, 1, C)], [(0, 1, 0)])
+    assert e.value.status == B.E3_ERR_BAD_PATH
+    with pytest.raises(B.E3Error) as e:        # l > 3
+        B.e3_jit_check([(4, 1, C)], 1, [(4, 1, C)], [(0, 0, 0)])
+    assert e.value.status == B.E3_ERR_UNSUPPORTED
+    with pytest.raises(B.E3Error) as e:        # unequal multiplicities
+        B.e3_jit_check([(0, 1, C), (1, -1, 2 * C)], 1, [(0, 1, C)], [(0, 0, 0)])
+    assert e.value.status == B.E3_ERR_UNSUPPORTED
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-device behaviour")
+def test_plan_create_fails_loudly_without_a_device():
+    with pytest.raises(B.E3Error) as e:
+        B.e3_plan_create([(0, 1, 4)], 0, [(0, 1, 4)], [(0, 0, 0)])
+    assert e.value.status == B.E3_ERR_CUDA
+    assert "no CPU fallback" in str(e.value)
+
+
+def test_product_package_never_imports_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2605_22698_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cpp", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src and "e3_oracle" not in src, f
