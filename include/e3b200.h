@@ -155,6 +155,11 @@ int e3_tp_scatter_bwd(const e3_plan *plan, const void *feats, const void *sh, co
                       const float *grad_out, float *grad_feats, float *grad_sh, void *grad_weights,
                       void *workspace, size_t workspace_bytes, e3_stream stream);
 
+/* Profiling aid (used by bench.py only): if `cuda_event` (a cudaEvent_t, or NULL to clear) is set,
+ * e3_tp_scatter_bwd records it on its stream between its two kernels, so that the dominant first
+ * phase and the per-sender reduction can be timed separately with CUDA events.  Not thread-safe. */
+int e3_profile_set_mid_event(e3_plan *plan, void *cuda_event);
+
 /* ---------------------------------------------------------------------------------------------
  * Edge -> atom force reduction (reading A10: vec_e = pos[rcv] - pos[snd] + shift):
  *   forces[i,:] = -( sum_{e : receivers[e]=i} grad_vec[e,:] - sum_{e : senders[e]=i} grad_vec[e,:] )

@@ -22,7 +22,7 @@ SYMBOLS = [
     "e3_status_string", "e3_last_error", "e3_all_paths", "e3_plan_create", "e3_plan_destroy", "e3_plan_dims",
     "e3_plan_get_cg", "e3_plan_kernel_info", "e3_plan_work", "e3_jit_check", "e3_graph_workspace_bytes",
     "e3_graph_prepare", "e3_sh_fwd", "e3_sh_bwd", "e3_tp_scatter_fwd", "e3_bwd_workspace_bytes", "e3_tp_scatter_bwd",
-    "e3_force_reduce", "e3_session_create", "e3_session_destroy", "e3_session_run_host",
+    "e3_force_reduce", "e3_profile_set_mid_event", "e3_session_create", "e3_session_destroy", "e3_session_run_host",
 ]
 
 
@@ -135,6 +135,11 @@ class Plan:
         cf = (C.c_double * n.value)()
         _check(lib().e3_plan_get_cg(self.handle, path, m1, m2, m3, cf, C.byref(n)), "e3_plan_get_cg")
         return list(zip(m1, m2, m3, cf))
+
+    def set_mid_event(self, event):
+        """Profiling aid: `event` is a recorded-once torch.cuda.Event(enable_timing=True) or None."""
+        h = C.c_void_p(event.cuda_event) if event is not None else C.c_void_p(0)
+        _check(lib().e3_profile_set_mid_event(self.handle, h), "e3_profile_set_mid_event")
 
     def destroy(self):
         if self.handle:

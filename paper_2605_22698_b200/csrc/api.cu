@@ -249,7 +249,15 @@ extern "C" int e3_tp_scatter_bwd(const e3_plan *plan, const void *feats, const v
                          (void *)&dxe, (void *)&grad_sh, (void *)&grad_weights, (void *)&ne };
         E3_CUDA_TRY(cudaLaunchKernel((const void *)plan->bwd.fn, dim3((unsigned)grid), dim3(plan->bwd.threads), args, 0, S(stream)));
     }
+    if (plan->mid_event) E3_CUDA_TRY(cudaEventRecord(plan->mid_event, S(stream)));
     return launch_dx_reduce(dxe, perm_s, col_ptr, n_nodes, plan->in_dim * plan->C, grad_feats, S(stream));
+}
+
+extern "C" int e3_profile_set_mid_event(e3_plan *plan, void *cuda_event)
+{
+    if (!plan) { set_error("plan is NULL"); return E3_ERR_INVALID_ARG; }
+    plan->mid_event = reinterpret_cast<cudaEvent_t>(cuda_event);
+    return E3_OK;
 }
 
 // ---------------------------------------------------------------------------------------------

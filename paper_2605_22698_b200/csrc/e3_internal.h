@@ -67,6 +67,7 @@ struct e3_plan {
     std::vector<e3::Role> roles;
     int fwd_warps = 4, bwd_warps = 4, bwd_edges_per_warp = 8;
     e3::JitKernel fwd, bwd;
+    cudaEvent_t mid_event = nullptr;   // profiling aid, see e3_profile_set_mid_event
 };
 
 namespace e3 {
