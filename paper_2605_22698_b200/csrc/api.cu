@@ -64,6 +64,12 @@ extern "C" int e3_plan_create(e3_plan **plan, const e3_irrep *irreps_in, int n_i
     if (rc == E3_OK) rc = plan_generate(*pl, nullptr);
     if (rc == E3_OK) rc = jit_load(pl->fwd);
     if (rc == E3_OK) rc = jit_load(pl->bwd);
+    if (rc == E3_OK && pl->fwd.smem_dyn > 48 * 1024 &&
+        cudaFuncSetAttribute((const void *)pl->fwd.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, pl->fwd.smem_dyn) != cudaSuccess)
+        rc = cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(fwd smem)");
+    if (rc == E3_OK && pl->bwd.smem_dyn > 48 * 1024 &&
+        cudaFuncSetAttribute((const void *)pl->bwd.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, pl->bwd.smem_dyn) != cudaSuccess)
+        rc = cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(bwd smem)");
     if (rc != E3_OK) { jit_unload(pl->fwd); jit_unload(pl->bwd); delete pl; return rc; }
     *plan = pl;
     return E3_OK;
@@ -106,7 +112,7 @@ extern "C" int e3_plan_kernel_info(const e3_plan *plan, int which, int *regs, in
     const JitKernel &k = which == 0 ? plan->fwd : plan->bwd;
     if (regs) *regs = k.regs;
     if (spill_bytes) *spill_bytes = k.spill;
-    if (smem_bytes) *smem_bytes = k.smem;
+    if (smem_bytes) *smem_bytes = k.smem + k.smem_dyn;
     if (threads_per_block) *threads_per_block = k.threads;
     if (n_roles) *n_roles = which == 0 ? (int)plan->roles.size() : 1;
     if (channels_per_lane) *channels_per_lane = plan->K;
@@ -202,11 +208,12 @@ extern "C" int e3_tp_scatter_fwd(const e3_plan *plan, const void *feats, const v
     }
     if (n_nodes == 0) return E3_OK;
     if (!plan->fwd.fn) { set_error("plan has no loaded forward kernel"); return E3_ERR_CUDA; }
-    long long items = (long long)n_nodes * (long long)plan->roles.size() * plan->nchb;
-    long long grid = (items + plan->fwd_warps - 1) / plan->fwd_warps;
+    const long long per_chunk = (long long)plan->fwd_chunk * plan->fwd_warps;     // receivers per chunk
+    const long long chunks = (n_nodes + per_chunk - 1) / per_chunk;
+    long long grid = chunks * plan->fwd_chunk * (long long)plan->roles.size() * plan->nchb;
     if (grid > 0x7fffffffLL) { set_error("grid too large"); return E3_ERR_UNSUPPORTED; }
     void *args[] = { (void *)&feats, (void *)&sh, (void *)&weights, (void *)&senders, (void *)&row_ptr, (void *)&out, (void *)&n_nodes };
-    E3_CUDA_TRY(cudaLaunchKernel((const void *)plan->fwd.fn, dim3((unsigned)grid), dim3(plan->fwd.threads), args, 0, S(stream)));
+    E3_CUDA_TRY(cudaLaunchKernel((const void *)plan->fwd.fn, dim3((unsigned)grid), dim3(plan->fwd.threads), args, plan->fwd.smem_dyn, S(stream)));
     return E3_OK;
 }
 
@@ -247,7 +254,7 @@ extern "C" int e3_tp_scatter_bwd(const e3_plan *plan, const void *feats, const v
         long long ne = n_edges;
         void *args[] = { (void *)&feats, (void *)&sh, (void *)&weights, (void *)&senders, (void *)&receivers, (void *)&grad_out,
                          (void *)&dxe, (void *)&grad_sh, (void *)&grad_weights, (void *)&ne };
-        E3_CUDA_TRY(cudaLaunchKernel((const void *)plan->bwd.fn, dim3((unsigned)grid), dim3(plan->bwd.threads), args, 0, S(stream)));
+        E3_CUDA_TRY(cudaLaunchKernel((const void *)plan->bwd.fn, dim3((unsigned)grid), dim3(plan->bwd.threads), args, plan->bwd.smem_dyn, S(stream)));
     }
     if (plan->mid_event) E3_CUDA_TRY(cudaEventRecord(plan->mid_event, S(stream)));
     return launch_dx_reduce(dxe, perm_s, col_ptr, n_nodes, plan->in_dim * plan->C, grad_feats, S(stream));

@@ -49,6 +49,7 @@ struct JitKernel {
     std::string source;
     std::vector<char> cubin;
     int regs = 0, spill = 0, smem = 0, threads = 0;
+    int smem_dyn = 0;          // dynamic shared memory per CTA (operand rings)
     cudaLibrary_t lib = nullptr;
     cudaKernel_t fn = nullptr;
 };
@@ -65,7 +66,11 @@ struct e3_plan {
     int K = 1;                 // channels per lane
     int nchb = 1;              // channel blocks of 32*K
     std::vector<e3::Role> roles;
-    int fwd_warps = 4, bwd_warps = 4, bwd_edges_per_warp = 8;
+    int fwd_warps = 4, bwd_warps = 4, bwd_edges_per_warp = 16;
+    int ring = 0;              // 1: cp.async operand rings, 0: plain loads (odd shapes)
+    int fwd_depth = 4, bwd_depth = 2;      // ring stages (fwd_depth must be a power of two)
+    int fwd_chunk = 512;       // CTAs per (chunk, role): CTA order is chunk-major, then role
+    int fwd_minb = 4, bwd_minb = 2;        // __launch_bounds__ min blocks per SM
     e3::JitKernel fwd, bwd;
     cudaEvent_t mid_event = nullptr;   // profiling aid, see e3_profile_set_mid_event
 };
@@ -79,8 +84,8 @@ int plan_build_tables(e3_plan &pl, const e3_irrep *irreps_in, int n_in, int sh_l
 void plan_make_roles(e3_plan &pl);
 
 // codegen.cpp
-std::string gen_forward_source(const e3_plan &pl);
-std::string gen_backward_source(const e3_plan &pl);
+std::string gen_forward_source(e3_plan &pl);    // also sets pl.fwd.smem_dyn
+std::string gen_backward_source(e3_plan &pl);   // also sets pl.bwd.smem_dyn
 
 // jit.cpp
 int jit_compile(JitKernel &k, const std::string &file_hint);   // NVRTC -> cubin (+regs/spill from the ptxas log)

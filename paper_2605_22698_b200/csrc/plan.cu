@@ -304,6 +304,8 @@ void plan_make_roles(e3_plan &pl)
     // channels per lane / channel blocks
     pl.K = (pl.C % 64 == 0) ? 2 : 1;
     pl.nchb = (pl.C + 32 * pl.K - 1) / (32 * pl.K);
+    const int slot_bytes = pl.K * (pl.dtype == E3_BF16 ? 2 : 4);
+    pl.ring = (pl.C % (32 * pl.K) == 0) && (slot_bytes == 4 || slot_bytes == 8);
 }
 
 }  // namespace e3
