@@ -230,9 +230,9 @@ extern "C" int e3_tp_scatter_bwd(const e3_plan *plan, const void *feats, const v
                                  float *grad_feats, float *grad_sh, void *grad_weights, void *workspace, size_t workspace_bytes,
                                  e3_stream stream)
 {
-    (void)row_ptr;
-    if (!plan || n_edges < 0 || n_nodes < 0 || !col_ptr || (n_nodes > 0 && (!feats || !grad_out || !grad_feats)) ||
-        (n_edges > 0 && (!sh || !weights || !senders || !receivers || !perm_s || !grad_sh))) {
+    (void)receivers;
+    if (!plan || n_edges < 0 || n_nodes < 0 || !col_ptr || !row_ptr || (n_nodes > 0 && (!feats || !grad_out || !grad_feats)) ||
+        (n_edges > 0 && (!sh || !weights || !senders || !perm_s || !grad_sh))) {
         set_error("e3_tp_scatter_bwd: bad arguments");
         return E3_ERR_INVALID_ARG;
     }
@@ -249,12 +249,10 @@ extern "C" int e3_tp_scatter_bwd(const e3_plan *plan, const void *feats, const v
     if (!plan->bwd.fn) { set_error("plan has no loaded backward kernel"); return E3_ERR_CUDA; }
     float *dxe = (float *)workspace;
     if (n_edges > 0) {
-        long long warps = (n_edges + plan->bwd_edges_per_warp - 1) / plan->bwd_edges_per_warp;
-        long long grid = (warps + plan->bwd_warps - 1) / plan->bwd_warps;
-        long long ne = n_edges;
-        void *args[] = { (void *)&feats, (void *)&sh, (void *)&weights, (void *)&senders, (void *)&receivers, (void *)&grad_out,
-                         (void *)&dxe, (void *)&grad_sh, (void *)&grad_weights, (void *)&ne };
-        E3_CUDA_TRY(cudaLaunchKernel((const void *)plan->bwd.fn, dim3((unsigned)grid), dim3(plan->bwd.threads), args, plan->bwd.smem_dyn, S(stream)));
+        // one CTA per receiver; its warps split the receiver's edges
+        void *args[] = { (void *)&feats, (void *)&sh, (void *)&weights, (void *)&senders, (void *)&row_ptr, (void *)&grad_out,
+                         (void *)&dxe, (void *)&grad_sh, (void *)&grad_weights, (void *)&n_nodes };
+        E3_CUDA_TRY(cudaLaunchKernel((const void *)plan->bwd.fn, dim3((unsigned)n_nodes), dim3(plan->bwd.threads), args, plan->bwd.smem_dyn, S(stream)));
     }
     if (plan->mid_event) E3_CUDA_TRY(cudaEventRecord(plan->mid_event, S(stream)));
     return launch_dx_reduce(dxe, perm_s, col_ptr, n_nodes, plan->in_dim * plan->C, grad_feats, S(stream));

@@ -66,9 +66,9 @@ struct e3_plan {
     int K = 1;                 // channels per lane
     int nchb = 1;              // channel blocks of 32*K
     std::vector<e3::Role> roles;
-    int fwd_warps = 4, bwd_warps = 4, bwd_edges_per_warp = 16;
+    int fwd_warps = 4, bwd_warps = 4;
     int ring = 0;              // 1: cp.async operand rings, 0: plain loads (odd shapes)
-    int fwd_depth = 4, bwd_depth = 2;      // ring stages (fwd_depth must be a power of two)
+    int fwd_depth = 4;         // forward ring stages (power of two); the backward ring has one rolling stage
     int fwd_chunk = 512;       // CTAs per (chunk, role): CTA order is chunk-major, then role
     int fwd_minb = 4, bwd_minb = 2;        // __launch_bounds__ min blocks per SM
     e3::JitKernel fwd, bwd;

@@ -4,8 +4,10 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <map>
+#include <string>
 
 #include "e3_internal.h"
 
@@ -282,7 +284,21 @@ void plan_make_roles(e3_plan &pl)
         total_cost += cost[o];
         total_rows += 2 * pl.irreps_out[o].l + 1;
     }
-    const int rows_target = 20, rows_hard = 28;
+    // tuning aid: E3_TUNE="key=value,..." overrides launch-shape heuristics (never changes results)
+    int rows_target = 20, rows_hard = 28;
+    if (const char *tune = getenv("E3_TUNE")) {
+        auto get = [&](const char *key, int &dst) {
+            std::string t(tune), k = std::string(key) + "=";
+            size_t pos = t.find(k);
+            if (pos != std::string::npos && (pos == 0 || t[pos - 1] == ',')) dst = atoi(t.c_str() + pos + k.size());
+        };
+        get("rows", rows_target); get("rows_hard", rows_hard);
+        get("fwd_minb", pl.fwd_minb); get("bwd_minb", pl.bwd_minb);
+        get("fwd_warps", pl.fwd_warps); get("bwd_warps", pl.bwd_warps);
+        get("fwd_depth", pl.fwd_depth);
+        get("chunk", pl.fwd_chunk);
+        if (rows_hard < rows_target) rows_hard = rows_target + 8;
+    }
     int n_roles = std::max(1, (total_rows + rows_target - 1) / rows_target);
     pl.roles.clear();
     Role cur; cur.rows = 0; cur.cost = 0.0;
@@ -305,7 +321,9 @@ void plan_make_roles(e3_plan &pl)
     pl.K = (pl.C % 64 == 0) ? 2 : 1;
     pl.nchb = (pl.C + 32 * pl.K - 1) / (32 * pl.K);
     const int slot_bytes = pl.K * (pl.dtype == E3_BF16 ? 2 : 4);
-    pl.ring = (pl.C % (32 * pl.K) == 0) && (slot_bytes == 4 || slot_bytes == 8);
+    // rings need 4/8-byte lane slots and 4-byte granular SH rows (bf16 with an odd sh_dim falls back to plain loads)
+    pl.ring = (pl.C % (32 * pl.K) == 0) && (slot_bytes == 4 || slot_bytes == 8) &&
+              ((pl.sh_dim * (pl.dtype == E3_BF16 ? 2 : 4)) % 4 == 0);
 }
 
 }  // namespace e3
