@@ -286,19 +286,15 @@ void plan_make_roles(e3_plan &pl)
     }
     // tuning aid: E3_TUNE="key=value,..." overrides launch-shape heuristics (never changes results)
     int rows_target = 20, rows_hard = 28;
-    if (const char *tune = getenv("E3_TUNE")) {
-        auto get = [&](const char *key, int &dst) {
-            std::string t(tune), k = std::string(key) + "=";
-            size_t pos = t.find(k);
-            if (pos != std::string::npos && (pos == 0 || t[pos - 1] == ',')) dst = atoi(t.c_str() + pos + k.size());
-        };
-        get("rows", rows_target); get("rows_hard", rows_hard);
-        get("fwd_minb", pl.fwd_minb); get("bwd_minb", pl.bwd_minb);
-        get("fwd_warps", pl.fwd_warps); get("bwd_warps", pl.bwd_warps);
-        get("fwd_depth", pl.fwd_depth);
-        get("chunk", pl.fwd_chunk);
-        if (rows_hard < rows_target) rows_hard = rows_target + 8;
-    }
+    const char *tune = getenv("E3_TUNE");
+    auto tune_get = [&](const char *key, int &dst) {
+        if (!tune) return;
+        std::string t(tune), k = std::string(key) + "=";
+        size_t pos = t.find(k);
+        if (pos != std::string::npos && (pos == 0 || t[pos - 1] == ',')) dst = atoi(t.c_str() + pos + k.size());
+    };
+    tune_get("rows", rows_target); tune_get("rows_hard", rows_hard);
+    if (rows_hard < rows_target) rows_hard = rows_target + 8;
     int n_roles = std::max(1, (total_rows + rows_target - 1) / rows_target);
     pl.roles.clear();
     Role cur; cur.rows = 0; cur.cost = 0.0;
@@ -324,6 +320,14 @@ void plan_make_roles(e3_plan &pl)
     // rings need 4/8-byte lane slots and 4-byte granular SH rows (bf16 with an odd sh_dim falls back to plain loads)
     pl.ring = (pl.C % (32 * pl.K) == 0) && (slot_bytes == 4 || slot_bytes == 8) &&
               ((pl.sh_dim * (pl.dtype == E3_BF16 ? 2 : 4)) % 4 == 0);
+    // forward ring depth: roles with long per-edge bodies hide the load latency with fewer stages in
+    // flight (and a shallower ring leaves room for more resident CTAs)
+    pl.fwd_depth = (total_cost / std::max<size_t>(1, pl.roles.size()) >= 100.0) ? 2 : 4;
+    pl.fwd_minb = 4;
+    pl.bwd_minb = 3;           // gen_backward_source lowers it when the shared-memory footprint allows fewer CTAs
+    tune_get("fwd_minb", pl.fwd_minb); tune_get("bwd_minb", pl.bwd_minb);
+    tune_get("fwd_warps", pl.fwd_warps); tune_get("bwd_warps", pl.bwd_warps);
+    tune_get("fwd_depth", pl.fwd_depth); tune_get("chunk", pl.fwd_chunk);
 }
 
 }  // namespace e3
