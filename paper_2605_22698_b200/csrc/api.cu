@@ -36,7 +36,7 @@ static int plan_generate(e3_plan &pl, const char *src_path)
     plan_make_roles(pl);
     pl.fwd.name = "e3_fwd";
     pl.bwd.name = "e3_bwd";
-    pl.fwd.source = gen_forward_source(pl);
+    pl.fwd.source = pl.v2 ? gen_forward_v2(pl) : gen_forward_source(pl);
     pl.bwd.source = gen_backward_source(pl);
     pl.fwd.threads = pl.fwd_warps * 32;
     pl.bwd.threads = pl.bwd_warps * 32;
@@ -115,7 +115,7 @@ extern "C" int e3_plan_kernel_info(const e3_plan *plan, int which, int *regs, in
     if (smem_bytes) *smem_bytes = k.smem + k.smem_dyn;
     if (threads_per_block) *threads_per_block = k.threads;
     if (n_roles) *n_roles = which == 0 ? (int)plan->roles.size() : 1;
-    if (channels_per_lane) *channels_per_lane = plan->K;
+    if (channels_per_lane) *channels_per_lane = (which == 0 && plan->v2) ? 4 : plan->K;
     return E3_OK;
 }
 
@@ -210,7 +210,7 @@ extern "C" int e3_tp_scatter_fwd(const e3_plan *plan, const void *feats, const v
     if (!plan->fwd.fn) { set_error("plan has no loaded forward kernel"); return E3_ERR_CUDA; }
     const long long per_chunk = (long long)plan->fwd_chunk * plan->fwd_warps;     // receivers per chunk
     const long long chunks = (n_nodes + per_chunk - 1) / per_chunk;
-    long long grid = chunks * plan->fwd_chunk * (long long)plan->roles.size() * plan->nchb;
+    long long grid = chunks * plan->fwd_chunk * (long long)plan->roles.size() * (plan->v2 ? plan->nchb2 : plan->nchb);
     if (grid > 0x7fffffffLL) { set_error("grid too large"); return E3_ERR_UNSUPPORTED; }
     void *args[] = { (void *)&feats, (void *)&sh, (void *)&weights, (void *)&senders, (void *)&row_ptr, (void *)&out, (void *)&n_nodes };
     E3_CUDA_TRY(cudaLaunchKernel((const void *)plan->fwd.fn, dim3((unsigned)grid), dim3(plan->fwd.threads), args, plan->fwd.smem_dyn, S(stream)));

@@ -68,6 +68,9 @@ struct e3_plan {
     std::vector<e3::Role> roles;
     int fwd_warps = 4, bwd_warps = 4;
     int ring = 0;              // 1: cp.async operand rings, 0: plain loads (odd shapes)
+    int v2 = 0;                // 1: second-generation kernels (factored form, 4 channels per lane, codegen2.cpp)
+    int lpe = 32, eps = 1;     // v2: lanes per edge (C/4, at most 32) and edges per warp step (32/lpe)
+    int nchb2 = 1;             // v2: channel blocks of 128
     int fwd_depth = 4;         // forward ring stages (power of two); the backward ring has one rolling stage
     int fwd_chunk = 512;       // CTAs per (chunk, role): CTA order is chunk-major, then role
     int fwd_minb = 4, bwd_minb = 2;        // __launch_bounds__ min blocks per SM
@@ -86,6 +89,10 @@ void plan_make_roles(e3_plan &pl);
 // codegen.cpp
 std::string gen_forward_source(e3_plan &pl);    // also sets pl.fwd.smem_dyn
 std::string gen_backward_source(e3_plan &pl);   // also sets pl.bwd.smem_dyn
+
+// codegen2.cpp (second generation; used when v2_eligible)
+bool v2_eligible(const e3_plan &pl);
+std::string gen_forward_v2(e3_plan &pl);
 
 // jit.cpp
 int jit_compile(JitKernel &k, const std::string &file_hint);   // NVRTC -> cubin (+regs/spill from the ptxas log)

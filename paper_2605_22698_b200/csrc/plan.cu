@@ -272,6 +272,7 @@ void plan_make_roles(e3_plan &pl)
     std::vector<int> order;
     for (int o = 0; o < n_out; ++o) if (!feeding[o].empty()) order.push_back(o);
     std::sort(order.begin(), order.end(), [&](int a, int b) { return first[a] < first[b]; });
+    for (int o = 0; o < n_out; ++o) if (feeding[o].empty()) order.push_back(o);   // unfed blocks are still written (zeros)
     std::vector<double> cost(n_out, 0.0);
     double total_cost = 0.0;
     int total_rows = 0;
@@ -285,7 +286,9 @@ void plan_make_roles(e3_plan &pl)
         total_rows += 2 * pl.irreps_out[o].l + 1;
     }
     // tuning aid: E3_TUNE="key=value,..." overrides launch-shape heuristics (never changes results)
-    int rows_target = 20, rows_hard = 28;
+    pl.v2 = v2_eligible(pl) ? 1 : 0;
+    { const char *t = getenv("E3_TUNE"); if (t && strstr(t, "v2=0")) pl.v2 = 0; }
+    int rows_target = pl.v2 ? 16 : 20, rows_hard = pl.v2 ? 22 : 28;
     const char *tune = getenv("E3_TUNE");
     auto tune_get = [&](const char *key, int &dst) {
         if (!tune) return;
@@ -325,6 +328,13 @@ void plan_make_roles(e3_plan &pl)
     pl.fwd_depth = (total_cost / std::max<size_t>(1, pl.roles.size()) >= 100.0) ? 2 : 4;
     pl.fwd_minb = 4;
     pl.bwd_minb = 3;           // gen_backward_source lowers it when the shared-memory footprint allows fewer CTAs
+    if (pl.v2) {               // second-generation kernels: 4 channels per lane, EPS edges per warp step
+        pl.lpe = pl.C >= 128 ? 32 : pl.C / 4;
+        pl.eps = 32 / pl.lpe;
+        pl.nchb2 = pl.C >= 128 ? pl.C / 128 : 1;
+        pl.fwd_depth = pl.eps >= 2 ? 2 : 3;
+        pl.fwd_minb = 3;
+    }
     tune_get("fwd_minb", pl.fwd_minb); tune_get("bwd_minb", pl.bwd_minb);
     tune_get("fwd_warps", pl.fwd_warps); tune_get("bwd_warps", pl.bwd_warps);
     tune_get("fwd_depth", pl.fwd_depth); tune_get("chunk", pl.fwd_chunk);
