@@ -37,7 +37,7 @@ static int plan_generate(e3_plan &pl, const char *src_path)
     pl.fwd.name = "e3_fwd";
     pl.bwd.name = "e3_bwd";
     pl.fwd.source = pl.v2 ? gen_forward_v2(pl) : gen_forward_source(pl);
-    pl.bwd.source = gen_backward_source(pl);
+    pl.bwd.source = pl.bwd_v2 ? gen_backward_v2(pl) : gen_backward_source(pl);
     pl.fwd.threads = pl.fwd_warps * 32;
     pl.bwd.threads = pl.bwd_warps * 32;
     std::string f1, f2;
@@ -70,6 +70,14 @@ extern "C" int e3_plan_create(e3_plan **plan, const e3_irrep *irreps_in, int n_i
     if (rc == E3_OK && pl->bwd.smem_dyn > 48 * 1024 &&
         cudaFuncSetAttribute((const void *)pl->bwd.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, pl->bwd.smem_dyn) != cudaSuccess)
         rc = cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(bwd smem)");
+    if (rc == E3_OK) {
+        int dev = 0, nsm = 0, a = 0, b = 0;
+        cudaGetDevice(&dev);
+        if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && nsm > 0) pl->n_sm = nsm;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, (const void *)pl->fwd.fn, pl->fwd.threads, pl->fwd.smem_dyn) == cudaSuccess && a > 0) pl->fwd_ctas_per_sm = a;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, (const void *)pl->bwd.fn, pl->bwd.threads, pl->bwd.smem_dyn) == cudaSuccess && b > 0) pl->bwd_ctas_per_sm = b;
+        cudaGetLastError();
+    }
     if (rc != E3_OK) { jit_unload(pl->fwd); jit_unload(pl->bwd); delete pl; return rc; }
     *plan = pl;
     return E3_OK;
@@ -115,7 +123,7 @@ extern "C" int e3_plan_kernel_info(const e3_plan *plan, int which, int *regs, in
     if (smem_bytes) *smem_bytes = k.smem + k.smem_dyn;
     if (threads_per_block) *threads_per_block = k.threads;
     if (n_roles) *n_roles = which == 0 ? (int)plan->roles.size() : 1;
-    if (channels_per_lane) *channels_per_lane = (which == 0 && plan->v2) ? 4 : plan->K;
+    if (channels_per_lane) *channels_per_lane = ((which == 0 && plan->v2) || (which == 1 && plan->bwd_v2)) ? 4 : plan->K;
     return E3_OK;
 }
 
@@ -208,11 +216,25 @@ extern "C" int e3_tp_scatter_fwd(const e3_plan *plan, const void *feats, const v
     }
     if (n_nodes == 0) return E3_OK;
     if (!plan->fwd.fn) { set_error("plan has no loaded forward kernel"); return E3_ERR_CUDA; }
-    const long long per_chunk = (long long)plan->fwd_chunk * plan->fwd_warps;     // receivers per chunk
+    // small graphs (v2 kernels): `fsplit` warps share one (receiver, role) so that the grid covers the machine
+    // several times over; the result depends on fsplit only through the (fixed) summation grouping
+    int fsplit = 1;
+    const long long nchb = plan->v2 ? plan->nchb2 : plan->nchb;
+    if (plan->v2) {
+        fsplit = plan->fwd_split;
+        if (fsplit <= 0) {
+            const double waves = (double)n_nodes * plan->roles.size() * nchb /
+                                 ((double)plan->n_sm * plan->fwd_ctas_per_sm * plan->fwd_warps);
+            fsplit = waves >= 6.0 ? 1 : (waves >= 3.0 ? 2 : 4);
+        }
+        if (fsplit != 1 && fsplit != 2 && fsplit != 4) fsplit = 1;
+        while (plan->fwd_warps % fsplit) fsplit >>= 1;
+    }
+    const long long per_chunk = (long long)plan->fwd_chunk * (plan->fwd_warps / fsplit);     // receivers per chunk
     const long long chunks = (n_nodes + per_chunk - 1) / per_chunk;
-    long long grid = chunks * plan->fwd_chunk * (long long)plan->roles.size() * (plan->v2 ? plan->nchb2 : plan->nchb);
+    long long grid = chunks * plan->fwd_chunk * (long long)plan->roles.size() * nchb;
     if (grid > 0x7fffffffLL) { set_error("grid too large"); return E3_ERR_UNSUPPORTED; }
-    void *args[] = { (void *)&feats, (void *)&sh, (void *)&weights, (void *)&senders, (void *)&row_ptr, (void *)&out, (void *)&n_nodes };
+    void *args[] = { (void *)&feats, (void *)&sh, (void *)&weights, (void *)&senders, (void *)&row_ptr, (void *)&out, (void *)&n_nodes, (void *)&fsplit };
     E3_CUDA_TRY(cudaLaunchKernel((const void *)plan->fwd.fn, dim3((unsigned)grid), dim3(plan->fwd.threads), args, plan->fwd.smem_dyn, S(stream)));
     return E3_OK;
 }
@@ -249,10 +271,22 @@ extern "C" int e3_tp_scatter_bwd(const e3_plan *plan, const void *feats, const v
     if (!plan->bwd.fn) { set_error("plan has no loaded backward kernel"); return E3_ERR_CUDA; }
     float *dxe = (float *)workspace;
     if (n_edges > 0) {
-        // one CTA per receiver; its warps split the receiver's edges
+        // one CTA per (receiver, part); its warps split the receiver's edges.  Small graphs are cut into `split`
+        // parts per receiver so that the grid still covers the machine several times over (tail effect).
+        int split = 1;
+        if (plan->bwd_v2) {
+            split = plan->bwd_split;
+            if (split <= 0) {
+                const long long slots = (long long)plan->n_sm * plan->bwd_ctas_per_sm;
+                split = (int)((8 * slots + n_nodes - 1) / n_nodes);
+                split = split < 1 ? 1 : (split > 4 ? 4 : split);
+            }
+        }
+        const long long grid = (long long)n_nodes * split;
+        if (grid > 0x7fffffffLL) { set_error("grid too large"); return E3_ERR_UNSUPPORTED; }
         void *args[] = { (void *)&feats, (void *)&sh, (void *)&weights, (void *)&senders, (void *)&row_ptr, (void *)&grad_out,
-                         (void *)&dxe, (void *)&grad_sh, (void *)&grad_weights, (void *)&n_nodes };
-        E3_CUDA_TRY(cudaLaunchKernel((const void *)plan->bwd.fn, dim3((unsigned)n_nodes), dim3(plan->bwd.threads), args, plan->bwd.smem_dyn, S(stream)));
+                         (void *)&dxe, (void *)&grad_sh, (void *)&grad_weights, (void *)&n_nodes, (void *)&split };
+        E3_CUDA_TRY(cudaLaunchKernel((const void *)plan->bwd.fn, dim3((unsigned)grid), dim3(plan->bwd.threads), args, plan->bwd.smem_dyn, S(stream)));
     }
     if (plan->mid_event) E3_CUDA_TRY(cudaEventRecord(plan->mid_event, S(stream)));
     return launch_dx_reduce(dxe, perm_s, col_ptr, n_nodes, plan->in_dim * plan->C, grad_feats, S(stream));

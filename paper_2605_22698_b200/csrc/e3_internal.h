@@ -74,6 +74,12 @@ struct e3_plan {
     int fwd_depth = 4;         // forward ring stages (power of two); the backward ring has one rolling stage
     int fwd_chunk = 512;       // CTAs per (chunk, role): CTA order is chunk-major, then role
     int fwd_minb = 4, bwd_minb = 2;        // __launch_bounds__ min blocks per SM
+    int bwd_v2 = 0;            // 1: second-generation backward (codegen2.cpp)
+    int bwd_r = 0;             // v2 backward: weights ring holds 1/bwd_r of a unit (0 = choose; set by the generator)
+    int bwd_split = 0;         // v2 backward: CTAs per receiver (0 = choose at launch from the grid size)
+    int fwd_split = 0;         // v2 forward: warps sharing one (receiver, role) (0 = choose at launch)
+    int fwd_ctas_per_sm = 2, bwd_ctas_per_sm = 2;   // measured residency (occupancy API) of the loaded kernels
+    int n_sm = 148;            // SM count of the device the plan was created on
     e3::JitKernel fwd, bwd;
     cudaEvent_t mid_event = nullptr;   // profiling aid, see e3_profile_set_mid_event
 };
@@ -93,6 +99,7 @@ std::string gen_backward_source(e3_plan &pl);   // also sets pl.bwd.smem_dyn
 // codegen2.cpp (second generation; used when v2_eligible)
 bool v2_eligible(const e3_plan &pl);
 std::string gen_forward_v2(e3_plan &pl);
+std::string gen_backward_v2(e3_plan &pl);  // also sets pl.bwd.smem_dyn, pl.bwd_r
 
 // jit.cpp
 int jit_compile(JitKernel &k, const std::string &file_hint);   // NVRTC -> cubin (+regs/spill from the ptxas log)

@@ -334,7 +334,11 @@ void plan_make_roles(e3_plan &pl)
         pl.nchb2 = pl.C >= 128 ? pl.C / 128 : 1;
         pl.fwd_depth = pl.eps >= 2 ? 2 : 3;
         pl.fwd_minb = 3;
+        pl.bwd_v2 = 1;
+        pl.bwd_minb = 2;
     }
+    tune_get("bwd_v2", pl.bwd_v2); tune_get("bwd_r", pl.bwd_r); tune_get("bwd_split", pl.bwd_split); tune_get("fwd_split", pl.fwd_split);
+    if (!pl.v2) pl.bwd_v2 = 0;
     tune_get("fwd_minb", pl.fwd_minb); tune_get("bwd_minb", pl.bwd_minb);
     tune_get("fwd_warps", pl.fwd_warps); tune_get("bwd_warps", pl.bwd_warps);
     tune_get("fwd_depth", pl.fwd_depth); tune_get("chunk", pl.fwd_chunk);
