@@ -243,7 +243,9 @@ extern "C" size_t e3_bwd_workspace_bytes(const e3_plan *plan, int64_t n_edges, i
 {
     (void)n_nodes;
     if (!plan || n_edges < 0) return 0;
-    return (size_t)n_edges * plan->in_dim * plan->C * sizeof(float) + 256;
+    size_t b = (size_t)n_edges * plan->in_dim * plan->C * sizeof(float) + 256;     // per-edge grad_feats rows
+    if (plan->bwd_v2 && plan->bwd_nroles > 1) b += (size_t)plan->bwd_nroles * n_edges * plan->sh_dim * sizeof(float) + 256;   // per-role grad_sh
+    return b;
 }
 
 extern "C" int e3_tp_scatter_bwd(const e3_plan *plan, const void *feats, const void *sh, const void *weights,
@@ -270,6 +272,8 @@ extern "C" int e3_tp_scatter_bwd(const e3_plan *plan, const void *feats, const v
     if (n_nodes == 0) return E3_OK;
     if (!plan->bwd.fn) { set_error("plan has no loaded backward kernel"); return E3_ERR_CUDA; }
     float *dxe = (float *)workspace;
+    float *gsh_parts = nullptr;
+    const int roles = plan->bwd_v2 ? plan->bwd_nroles : 1;
     if (n_edges > 0) {
         // one CTA per (receiver, part); its warps split the receiver's edges.  Small graphs are cut into `split`
         // parts per receiver so that the grid still covers the machine several times over (tail effect).
@@ -282,14 +286,26 @@ extern "C" int e3_tp_scatter_bwd(const e3_plan *plan, const void *feats, const v
                 split = split < 1 ? 1 : (split > 4 ? 4 : split);
             }
         }
-        const long long grid = (long long)n_nodes * split;
+        long long grid = (long long)n_nodes * split;
+        if (plan->bwd_v2) {           // CTA order: chunk of receivers, then role, then (receiver, part)
+            const long long chunks = ((long long)n_nodes + plan->bwd_chunk - 1) / plan->bwd_chunk;
+            grid = chunks * plan->bwd_chunk * plan->bwd_nroles * split;
+        }
         if (grid > 0x7fffffffLL) { set_error("grid too large"); return E3_ERR_UNSUPPORTED; }
+        if (roles > 1) {
+            const size_t off = (((size_t)n_edges * plan->in_dim * plan->C * sizeof(float) + 255) / 256) * 256;
+            gsh_parts = reinterpret_cast<float *>(reinterpret_cast<char *>(workspace) + off);
+        }
+        float *gsh_arg = roles > 1 ? gsh_parts : grad_sh;
+        long long ne = n_edges;
         void *args[] = { (void *)&feats, (void *)&sh, (void *)&weights, (void *)&senders, (void *)&row_ptr, (void *)&grad_out,
-                         (void *)&dxe, (void *)&grad_sh, (void *)&grad_weights, (void *)&n_nodes, (void *)&split };
+                         (void *)&dxe, (void *)&gsh_arg, (void *)&grad_weights, (void *)&n_nodes, (void *)&split, (void *)&ne };
         E3_CUDA_TRY(cudaLaunchKernel((const void *)plan->bwd.fn, dim3((unsigned)grid), dim3(plan->bwd.threads), args, plan->bwd.smem_dyn, S(stream)));
     }
     if (plan->mid_event) E3_CUDA_TRY(cudaEventRecord(plan->mid_event, S(stream)));
-    return launch_dx_reduce(dxe, perm_s, col_ptr, n_nodes, plan->in_dim * plan->C, grad_feats, S(stream));
+    int rc = launch_dx_reduce(dxe, perm_s, col_ptr, n_nodes, plan->in_dim * plan->C, grad_feats, S(stream));
+    if (rc == E3_OK && roles > 1 && n_edges > 0) rc = launch_gsh_reduce(gsh_parts, roles, n_edges * plan->sh_dim, grad_sh, S(stream));
+    return rc;
 }
 
 extern "C" int e3_profile_set_mid_event(e3_plan *plan, void *cuda_event)

@@ -72,10 +72,15 @@ struct e3_plan {
     int lpe = 32, eps = 1;     // v2: lanes per edge (C/4, at most 32) and edges per warp step (32/lpe)
     int nchb2 = 1;             // v2: channel blocks of 128
     int fwd_depth = 4;         // forward ring stages (power of two); the backward ring has one rolling stage
+    int fwd_depth_max = 6;     // v2 forward: roles with small stages deepen their ring up to this many stages
     int fwd_chunk = 512;       // CTAs per (chunk, role): CTA order is chunk-major, then role
     int fwd_minb = 4, bwd_minb = 2;        // __launch_bounds__ min blocks per SM
     int bwd_v2 = 0;            // 1: second-generation backward (codegen2.cpp)
     int bwd_r = 0;             // v2 backward: weights ring holds 1/bwd_r of a unit (0 = choose; set by the generator)
+    int bwd_nroles = 1;        // v2 backward: roles (runs of input irreps) per receiver; grad_sh is summed over roles afterwards
+    int bwd_role_cost = 0;     // v2 backward: cost target of one role in packed operations (0 = default)
+    int bwd_chunk = 4096;      // v2 backward: receivers per chunk (CTA order is chunk-major, then role)
+    int bwd_depth = 0;         // v2 backward: ring stages per warp (units in flight); 0 = choose
     int bwd_split = 0;         // v2 backward: CTAs per receiver (0 = choose at launch from the grid size)
     int fwd_split = 0;         // v2 forward: warps sharing one (receiver, role) (0 = choose at launch)
     int fwd_ctas_per_sm = 2, bwd_ctas_per_sm = 2;   // measured residency (occupancy API) of the loaded kernels
@@ -116,6 +121,7 @@ int launch_force_reduce(const float *gvec, const int32_t *row_ptr, const int32_t
                         int64_t E, int32_t N, float *forces, cudaStream_t st);
 int launch_dx_reduce(const float *dxe, const int32_t *perm_s, const int32_t *col_ptr, int32_t N, int row_len,
                      float *dx, cudaStream_t st);
+int launch_gsh_reduce(const float *parts, int n_parts, int64_t n, float *gsh, cudaStream_t st);
 int launch_cg_planner(const int *triples /*[n,3] host*/, int n, std::vector<std::vector<double>> &dense_out);
 
 }  // namespace e3

@@ -335,6 +335,25 @@ __global__ void dx_reduce_kernel(const float *__restrict__ dxe, const int32_t *_
     }
 }
 
+// grad_sh = sum over the backward roles' partial buffers, in role order (deterministic)
+__global__ void gsh_reduce_kernel(const float *__restrict__ parts, int n_parts, long long n, float *__restrict__ gsh)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float acc = parts[i];
+    for (int k = 1; k < n_parts; ++k) acc += parts[(size_t)k * n + i];
+    gsh[i] = acc;
+}
+
+int launch_gsh_reduce(const float *parts, int n_parts, int64_t n, float *gsh, cudaStream_t st)
+{
+    if (n <= 0) return E3_OK;
+    const int th = 256;
+    gsh_reduce_kernel<<<(unsigned)((n + th - 1) / th), th, 0, st>>>(parts, n_parts, (long long)n, gsh);
+    E3_CUDA_TRY(cudaGetLastError());
+    return E3_OK;
+}
+
 int launch_dx_reduce(const float *dxe, const int32_t *perm_s, const int32_t *col_ptr, int32_t N, int row_len,
                      float *dx, cudaStream_t st)
 {

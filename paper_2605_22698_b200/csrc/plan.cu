@@ -288,7 +288,7 @@ void plan_make_roles(e3_plan &pl)
     // tuning aid: E3_TUNE="key=value,..." overrides launch-shape heuristics (never changes results)
     pl.v2 = v2_eligible(pl) ? 1 : 0;
     { const char *t = getenv("E3_TUNE"); if (t && strstr(t, "v2=0")) pl.v2 = 0; }
-    int rows_target = pl.v2 ? 16 : 20, rows_hard = pl.v2 ? 22 : 28;
+    int rows_target = 20, rows_hard = pl.v2 ? 22 : 28;
     const char *tune = getenv("E3_TUNE");
     auto tune_get = [&](const char *key, int &dst) {
         if (!tune) return;
@@ -337,7 +337,7 @@ void plan_make_roles(e3_plan &pl)
         pl.bwd_v2 = 1;
         pl.bwd_minb = 2;
     }
-    tune_get("bwd_v2", pl.bwd_v2); tune_get("bwd_r", pl.bwd_r); tune_get("bwd_split", pl.bwd_split); tune_get("fwd_split", pl.fwd_split);
+    tune_get("bwd_v2", pl.bwd_v2); tune_get("fwd_depth_max", pl.fwd_depth_max); tune_get("bwd_depth", pl.bwd_depth); tune_get("bwd_role_cost", pl.bwd_role_cost); tune_get("bwd_chunk", pl.bwd_chunk); tune_get("bwd_r", pl.bwd_r); tune_get("bwd_split", pl.bwd_split); tune_get("fwd_split", pl.fwd_split);
     if (!pl.v2) pl.bwd_v2 = 0;
     tune_get("fwd_minb", pl.fwd_minb); tune_get("bwd_minb", pl.bwd_minb);
     tune_get("fwd_warps", pl.fwd_warps); tune_get("bwd_warps", pl.bwd_warps);
