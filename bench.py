@@ -270,7 +270,8 @@ def run_ours(args):
         chk(L.e3_force_reduce(p(gvec), p(row_ptr), p(perm_s), p(col_ptr), Ct.c_int64(E), Ct.c_int32(N), p(F), sp), "e3_force_reduce")
         mark("force_reduce")
 
-    KERNELS_PER_STEP = 5 + 1 + 1 + 2 + 1 + 1     # graph(row_ptr,count,scan,fill,sort) sh_fwd fwd bwd+dx_reduce sh_bwd force
+    # graph(row_ptr,count,scan,fill,sort) sh_fwd fwd bwd+dx_reduce(+gsh_reduce when the backward has several roles) sh_bwd force
+    KERNELS_PER_STEP = 5 + 1 + 1 + 2 + (1 if plan.kernel_info(1)["n_roles"] > 1 else 0) + 1 + 1
 
     def barrier():
         if world > 1:
@@ -312,7 +313,7 @@ def run_ours(args):
         tb = [e for n_, e in evs if n_ == "tp_scatter_fwd"][0]
         te = [e for n_, e in evs if n_ == "tp_scatter_bwd"][0]
         acc.setdefault("e3_bwd_kernel", []).append(tb.elapsed_time(mid))
-        acc.setdefault("dx_reduce_kernel", []).append(mid.elapsed_time(te))
+        acc.setdefault("dx_reduce_kernel", []).append(mid.elapsed_time(te))     # + gsh_reduce when the backward has several roles
     plan.set_mid_event(None)
     kms = {k: float(np.mean(v)) for k, v in acc.items()}
 

@@ -122,7 +122,7 @@ extern "C" int e3_plan_kernel_info(const e3_plan *plan, int which, int *regs, in
     if (spill_bytes) *spill_bytes = k.spill;
     if (smem_bytes) *smem_bytes = k.smem + k.smem_dyn;
     if (threads_per_block) *threads_per_block = k.threads;
-    if (n_roles) *n_roles = which == 0 ? (int)plan->roles.size() : 1;
+    if (n_roles) *n_roles = which == 0 ? (int)plan->roles.size() : (plan->bwd_v2 ? plan->bwd_nroles : 1);
     if (channels_per_lane) *channels_per_lane = ((which == 0 && plan->v2) || (which == 1 && plan->bwd_v2)) ? 4 : plan->K;
     return E3_OK;
 }

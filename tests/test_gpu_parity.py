@@ -204,6 +204,42 @@ def test_vjp_with_arbitrary_sh_input_and_no_grad_weights():
     assert np.array_equal(dx.cpu().numpy(), gpu["dx"]) and np.array_equal(dY.cpu().numpy(), gpu["dY"])
 
 
+# ------------------------------------------------------------------ launch-shape variants of the generated kernels
+@pytest.mark.parametrize("tune", [
+    "fwd_split=1,bwd_split=1", "fwd_split=2,bwd_split=3", "fwd_split=4,bwd_split=4",       # warps / CTAs sharing a receiver
+    "bwd_role_cost=1", "bwd_role_cost=1000000",                                               # one role per input irrep / a single role
+    "bwd_depth=1", "bwd_depth=1,bwd_r=2", "bwd_depth=1,bwd_r=2,bwd_role_cost=1000000",        # ring stages, half-unit weights ring
+    "fwd_depth_max=2", "rows=12", "rows=20,rows_hard=30,fwd_minb=2", "chunk=3,bwd_chunk=5",   # forward ring depth, role sizes, CTA order
+    "bwd_v2=0", "v2=0",                                                                       # first-generation kernels
+])
+@pytest.mark.parametrize("C", [32, 64, 128])
+def test_launch_shape_variants(tune, C, monkeypatch):
+    """E3_TUNE only moves work between warps / CTAs / ring stages; every variant must meet the same parity bars.
+    C = 32 / 64 / 128 gives 4 / 2 / 1 edges per warp step; degrees 0..90 give ragged steps and empty parts."""
+    rng = np.random.default_rng(1000 + C)
+    cfg = W.small_config(channels=C, irreps_in=((0, 1), (1, -1), (2, 1), (3, -1)), sh_lmax=3, out_lmax=3)
+    pl = plan_inputs(cfg)
+    n = 23
+    deg = rng.integers(0, 12, size=n); deg[4] = 90; deg[9] = 0; deg[10] = 1; deg[11] = 33
+    rcv = np.repeat(np.arange(n), deg)
+    snd = rng.integers(0, n, size=rcv.size)
+    o = np.lexsort((snd, rcv))
+    snd, rcv = snd[o].astype(np.int32), rcv[o].astype(np.int32)
+    e = rcv.size
+    g = W.Graph(n, np.zeros((n, 3)), snd, rcv, (rng.normal(size=(e, 3)) * 2).astype(np.float32), 0.0)
+    x = rng.normal(size=(n, 16 * C)).astype(np.float32)
+    w = rng.normal(size=(e, 34 * C)).astype(np.float32)
+    G = rng.normal(size=(n, 156 * C)).astype(np.float32)
+    monkeypatch.setenv("E3_TUNE", tune)
+    plan = gpu_plan(pl)
+    monkeypatch.delenv("E3_TUNE")
+    gpu = run_gpu(plan, g, x, w, G)
+    compare(gpu, run_oracle(pl, g, x, w, G))
+    again = run_gpu(plan, g, x, w, G)
+    for k in gpu:
+        assert np.array_equal(gpu[k], again[k]), k
+
+
 # ------------------------------------------------------------------ bf16 storage (reading A12)
 def test_bf16_storage_parity_and_fp32_recovers():
     cfg = W.small_config(n_atoms=200, channels=128, irreps_in=((0, 1), (1, -1), (2, 1), (3, -1)), sh_lmax=3, out_lmax=3,
