@@ -261,7 +261,7 @@ extern "C" int e3_tp_scatter_bwd(const e3_plan *plan, const void *feats, const v
         return E3_ERR_INVALID_ARG;
     }
     if (!aligned16(feats) || !aligned16(weights) || !aligned16(grad_out) || !aligned16(grad_feats) || !aligned16(grad_weights) ||
-        !aligned16(sh) || !aligned16(workspace)) {
+        !aligned16(sh) || !aligned16(workspace) || !aligned16(grad_sh)) {
         set_error("e3_tp_scatter_bwd: tensor pointers must be 16-byte aligned");
         return E3_ERR_INVALID_ARG;
     }

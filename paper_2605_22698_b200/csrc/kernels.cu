@@ -304,52 +304,79 @@ template <int VEC>
 __global__ void dx_reduce_kernel(const float *__restrict__ dxe, const int32_t *__restrict__ perm_s,
                                  const int32_t *__restrict__ col_ptr, int row_len, float *__restrict__ dx)
 {
+    constexpr int TILE = 512, U = 8;            // edge ids staged per pass; rows in flight per thread
+    __shared__ int32_t eid[TILE];
     const int32_t s = blockIdx.x;
     const int32_t a = col_ptr[s], b = col_ptr[s + 1];
-    for (int c = threadIdx.x * VEC; c < row_len; c += blockDim.x * VEC) {
+    // each thread owns up to two column groups (row_len <= 2 * blockDim.x * VEC covers every plan up to l = 3, C = 128 * 4)
+    for (int c0 = 0; c0 < row_len; c0 += blockDim.x * VEC) {
+        const int c = c0 + threadIdx.x * VEC;
+        const bool act = c < row_len;
         float acc[VEC];
 #pragma unroll
         for (int v = 0; v < VEC; ++v) acc[v] = 0.0f;
-        int32_t j = a;
-        for (; j + 4 <= b; j += 4) {
-            float t[4][VEC];
+        for (int32_t t0 = a; t0 < b; t0 += TILE) {
+            const int nt = min(TILE, b - t0);
+            __syncthreads();
+            for (int i = threadIdx.x; i < nt; i += blockDim.x) eid[i] = perm_s[t0 + i];
+            __syncthreads();
+            if (act) {
+                int j = 0;
+                for (; j + U <= nt; j += U) {
+                    float t[U][VEC];
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const float *row = dxe + (size_t)perm_s[j + q] * row_len + c;
-                if constexpr (VEC == 4) { float4 v4 = *reinterpret_cast<const float4 *>(row); t[q][0] = v4.x; t[q][1] = v4.y; t[q][2] = v4.z; t[q][3] = v4.w; }
-                else t[q][0] = row[0];
+                    for (int q = 0; q < U; ++q) {
+                        const float *row = dxe + (size_t)eid[j + q] * row_len + c;
+                        if constexpr (VEC == 4) { float4 v4 = __ldcs(reinterpret_cast<const float4 *>(row)); t[q][0] = v4.x; t[q][1] = v4.y; t[q][2] = v4.z; t[q][3] = v4.w; }
+                        else t[q][0] = __ldcs(row);
+                    }
+#pragma unroll
+                    for (int q = 0; q < U; ++q)
+#pragma unroll
+                        for (int v = 0; v < VEC; ++v) acc[v] += t[q][v];
+                }
+                for (; j < nt; ++j) {
+                    const float *row = dxe + (size_t)eid[j] * row_len + c;
+#pragma unroll
+                    for (int v = 0; v < VEC; ++v) acc[v] += row[v];
+                }
             }
-#pragma unroll
-            for (int q = 0; q < 4; ++q)
-#pragma unroll
-                for (int v = 0; v < VEC; ++v) acc[v] += t[q][v];
         }
-        for (; j < b; ++j) {
-            const float *row = dxe + (size_t)perm_s[j] * row_len + c;
-#pragma unroll
-            for (int v = 0; v < VEC; ++v) acc[v] += row[v];
+        if (act) {
+            float *o = dx + (size_t)s * row_len + c;
+            if constexpr (VEC == 4) *reinterpret_cast<float4 *>(o) = make_float4(acc[0], acc[1], acc[2], acc[3]);
+            else o[0] = acc[0];
         }
-        float *o = dx + (size_t)s * row_len + c;
-        if constexpr (VEC == 4) *reinterpret_cast<float4 *>(o) = make_float4(acc[0], acc[1], acc[2], acc[3]);
-        else o[0] = acc[0];
     }
 }
 
 // grad_sh = sum over the backward roles' partial buffers, in role order (deterministic)
 __global__ void gsh_reduce_kernel(const float *__restrict__ parts, int n_parts, long long n, float *__restrict__ gsh)
 {
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    float acc = parts[i];
-    for (int k = 1; k < n_parts; ++k) acc += parts[(size_t)k * n + i];
-    gsh[i] = acc;
+    const long long i4 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 4;
+    if (i4 >= n) return;
+    if (i4 + 4 <= n && (n & 3) == 0) {           // part k starts at k * n floats: 16-byte aligned when n % 4 == 0
+        float4 acc = __ldcs(reinterpret_cast<const float4 *>(parts + i4));
+        for (int k = 1; k < n_parts; ++k) {
+            const float4 v = __ldcs(reinterpret_cast<const float4 *>(parts + (size_t)k * n + i4));
+            acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
+        }
+        *reinterpret_cast<float4 *>(gsh + i4) = acc;
+    } else {
+        for (long long i = i4; i < n && i < i4 + 4; ++i) {
+            float acc = parts[i];
+            for (int k = 1; k < n_parts; ++k) acc += parts[(size_t)k * n + i];
+            gsh[i] = acc;
+        }
+    }
 }
 
 int launch_gsh_reduce(const float *parts, int n_parts, int64_t n, float *gsh, cudaStream_t st)
 {
     if (n <= 0) return E3_OK;
     const int th = 256;
-    gsh_reduce_kernel<<<(unsigned)((n + th - 1) / th), th, 0, st>>>(parts, n_parts, (long long)n, gsh);
+    const long long n4 = (n + 3) / 4;
+    gsh_reduce_kernel<<<(unsigned)((n4 + th - 1) / th), th, 0, st>>>(parts, n_parts, (long long)n, gsh);
     E3_CUDA_TRY(cudaGetLastError());
     return E3_OK;
 }
