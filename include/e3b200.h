@@ -160,6 +160,13 @@ int e3_tp_scatter_bwd(const e3_plan *plan, const void *feats, const void *sh, co
  * phase and the per-sender reduction can be timed separately with CUDA events.  Not thread-safe. */
 int e3_profile_set_mid_event(e3_plan *plan, void *cuda_event);
 
+/* Measurement aid (used by bench.py only; SURVEY section 7 "FP32 peak is not in MEASURED_PEAKS.json"): runs a
+ * register-only packed-FMA kernel (8 independent FFMA2 chains per thread, one full wave of 1024-thread CTAs) for about
+ * `ms_target` milliseconds on `stream`, synchronises, and returns the achieved FP32 rate in TFLOP/s (2 flop per FMA lane)
+ * in *tflops.  It is the sustained FFMA ceiling of THIS board at the clock its power cap allows, reported beside the nominal
+ * 148 x 128 x 2 x 1.965 GHz peak that the roofline fractions use.  Returns E3_ERR_CUDA without a device. */
+int e3_measure_fp32_peak(double *tflops, double ms_target, e3_stream stream);
+
 /* ---------------------------------------------------------------------------------------------
  * Edge -> atom force reduction (reading A10: vec_e = pos[rcv] - pos[snd] + shift):
  *   forces[i,:] = -( sum_{e : receivers[e]=i} grad_vec[e,:] - sum_{e : senders[e]=i} grad_vec[e,:] )
@@ -171,9 +178,12 @@ int e3_force_reduce(const float *grad_vec /*[E,3]*/, const int32_t *row_ptr, con
 
 /* ---------------------------------------------------------------------------------------------
  * Host-buffer entry point: one pass of the whole hot path (a2..a7) with HOST inputs and outputs.
- * The session owns device buffers sized for (max_edges, max_nodes) and one stream; each run copies
- * the inputs host->device, runs graph_prepare, sh_fwd, tp_scatter_fwd, tp_scatter_bwd, sh_bwd and
- * force_reduce, copies the requested results device->host and synchronises.  Any output pointer
+ * The session owns device buffers sized for (max_edges, max_nodes), a compute stream and two copy
+ * streams; each run copies the inputs host->device, runs graph_prepare, sh_fwd, tp_scatter_fwd,
+ * tp_scatter_bwd, sh_bwd and force_reduce, copies the requested results device->host and synchronises.
+ * The weights / out / grad_weights traffic is pipelined over contiguous receiver ranges (copy-in of range
+ * k+1, compute of range k and copy-out of range k-1 overlap); results are bit-identical to the device
+ * entry points on the same inputs.  Host buffers should be pinned for the overlap.  Any output pointer
  * may be NULL (skipped, and its copy is not made).  Inputs have the plan's storage dtype where
  * the device entry points do.  bytes_h2d / bytes_d2h (may be NULL) receive the bytes copied.
  * -------------------------------------------------------------------------------------------*/

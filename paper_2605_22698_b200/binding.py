@@ -22,7 +22,7 @@ SYMBOLS = [
     "e3_status_string", "e3_last_error", "e3_all_paths", "e3_plan_create", "e3_plan_destroy", "e3_plan_dims",
     "e3_plan_get_cg", "e3_plan_kernel_info", "e3_plan_work", "e3_jit_check", "e3_graph_workspace_bytes",
     "e3_graph_prepare", "e3_sh_fwd", "e3_sh_bwd", "e3_tp_scatter_fwd", "e3_bwd_workspace_bytes", "e3_tp_scatter_bwd",
-    "e3_force_reduce", "e3_profile_set_mid_event", "e3_session_create", "e3_session_destroy", "e3_session_run_host",
+    "e3_force_reduce", "e3_profile_set_mid_event", "e3_measure_fp32_peak", "e3_session_create", "e3_session_destroy", "e3_session_run_host",
 ]
 
 
@@ -210,6 +210,13 @@ def e3_tp_scatter_fwd(plan: Plan, feats, sh, weights, senders, receivers, row_pt
                                    _ptr(row_ptr), C.c_int64(E), C.c_int32(n_nodes), _ptr(_dev(out, torch.float32)),
                                    _stream(stream)), "e3_tp_scatter_fwd")
     return out
+
+
+def e3_measure_fp32_peak(ms_target=200.0, stream=None):
+    """Sustained packed-FMA rate of this board in TFLOP/s (measurement aid, see include/e3b200.h)."""
+    t = C.c_double(0.0)
+    _check(lib().e3_measure_fp32_peak(C.byref(t), C.c_double(ms_target), _stream(stream)), "e3_measure_fp32_peak")
+    return float(t.value)
 
 
 def e3_bwd_workspace_bytes(plan: Plan, n_edges, n_nodes):

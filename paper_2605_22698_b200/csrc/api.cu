@@ -200,6 +200,37 @@ extern "C" int e3_force_reduce(const float *grad_vec, const int32_t *row_ptr, co
 // ---------------------------------------------------------------------------------------------
 // tensor product + scatter
 // ---------------------------------------------------------------------------------------------
+// launches the forward kernel for the receivers whose row_ptr / out rows start at the given pointers (a receiver range
+// of a larger graph is the same call with offset pointers: edge-indexed and sender-indexed tensors stay absolute)
+static int launch_fwd(const e3_plan *plan, const void *feats, const void *sh, const void *weights, const int32_t *senders,
+                      const int32_t *row_ptr, int32_t n_nodes, float *out, cudaStream_t st, int32_t heur_nodes = -1)
+{
+    if (heur_nodes < 0) heur_nodes = n_nodes;     // launch-shape heuristics follow the size of the WHOLE graph
+    if (n_nodes == 0) return E3_OK;
+    if (!plan->fwd.fn) { set_error("plan has no loaded forward kernel"); return E3_ERR_CUDA; }
+    // small graphs (v2 kernels): `fsplit` warps share one (receiver, role) so that the grid covers the machine
+    // several times over; the result depends on fsplit only through the (fixed) summation grouping
+    int fsplit = 1;
+    const long long nchb = plan->v2 ? plan->nchb2 : plan->nchb;
+    if (plan->v2) {
+        fsplit = plan->fwd_split;
+        if (fsplit <= 0) {
+            const double waves = (double)heur_nodes * plan->roles.size() * nchb /
+                                 ((double)plan->n_sm * plan->fwd_ctas_per_sm * plan->fwd_warps);
+            fsplit = waves >= 6.0 ? 1 : (waves >= 3.0 ? 2 : 4);
+        }
+        if (fsplit != 1 && fsplit != 2 && fsplit != 4) fsplit = 1;
+        while (plan->fwd_warps % fsplit) fsplit >>= 1;
+    }
+    const long long per_chunk = (long long)plan->fwd_chunk * (plan->fwd_warps / fsplit);     // receivers per chunk
+    const long long chunks = (n_nodes + per_chunk - 1) / per_chunk;
+    long long grid = chunks * plan->fwd_chunk * (long long)plan->roles.size() * nchb;
+    if (grid > 0x7fffffffLL) { set_error("grid too large"); return E3_ERR_UNSUPPORTED; }
+    void *args[] = { (void *)&feats, (void *)&sh, (void *)&weights, (void *)&senders, (void *)&row_ptr, (void *)&out, (void *)&n_nodes, (void *)&fsplit };
+    E3_CUDA_TRY(cudaLaunchKernel((const void *)plan->fwd.fn, dim3((unsigned)grid), dim3(plan->fwd.threads), args, plan->fwd.smem_dyn, st));
+    return E3_OK;
+}
+
 extern "C" int e3_tp_scatter_fwd(const e3_plan *plan, const void *feats, const void *sh, const void *weights,
                                  const int32_t *senders, const int32_t *receivers, const int32_t *row_ptr, int64_t n_edges,
                                  int32_t n_nodes, float *out, e3_stream stream)
@@ -214,38 +245,69 @@ extern "C" int e3_tp_scatter_fwd(const e3_plan *plan, const void *feats, const v
         set_error("e3_tp_scatter_fwd: tensor pointers must be 16-byte aligned");
         return E3_ERR_INVALID_ARG;
     }
-    if (n_nodes == 0) return E3_OK;
-    if (!plan->fwd.fn) { set_error("plan has no loaded forward kernel"); return E3_ERR_CUDA; }
-    // small graphs (v2 kernels): `fsplit` warps share one (receiver, role) so that the grid covers the machine
-    // several times over; the result depends on fsplit only through the (fixed) summation grouping
-    int fsplit = 1;
-    const long long nchb = plan->v2 ? plan->nchb2 : plan->nchb;
-    if (plan->v2) {
-        fsplit = plan->fwd_split;
-        if (fsplit <= 0) {
-            const double waves = (double)n_nodes * plan->roles.size() * nchb /
-                                 ((double)plan->n_sm * plan->fwd_ctas_per_sm * plan->fwd_warps);
-            fsplit = waves >= 6.0 ? 1 : (waves >= 3.0 ? 2 : 4);
-        }
-        if (fsplit != 1 && fsplit != 2 && fsplit != 4) fsplit = 1;
-        while (plan->fwd_warps % fsplit) fsplit >>= 1;
-    }
-    const long long per_chunk = (long long)plan->fwd_chunk * (plan->fwd_warps / fsplit);     // receivers per chunk
-    const long long chunks = (n_nodes + per_chunk - 1) / per_chunk;
-    long long grid = chunks * plan->fwd_chunk * (long long)plan->roles.size() * nchb;
-    if (grid > 0x7fffffffLL) { set_error("grid too large"); return E3_ERR_UNSUPPORTED; }
-    void *args[] = { (void *)&feats, (void *)&sh, (void *)&weights, (void *)&senders, (void *)&row_ptr, (void *)&out, (void *)&n_nodes, (void *)&fsplit };
-    E3_CUDA_TRY(cudaLaunchKernel((const void *)plan->fwd.fn, dim3((unsigned)grid), dim3(plan->fwd.threads), args, plan->fwd.smem_dyn, S(stream)));
-    return E3_OK;
+    return launch_fwd(plan, feats, sh, weights, senders, row_ptr, n_nodes, out, S(stream));
 }
 
 extern "C" size_t e3_bwd_workspace_bytes(const e3_plan *plan, int64_t n_edges, int32_t n_nodes)
 {
     (void)n_nodes;
     if (!plan || n_edges < 0) return 0;
-    size_t b = (size_t)n_edges * plan->in_dim * plan->C * sizeof(float) + 256;     // per-edge grad_feats rows
+    size_t b = (((size_t)n_edges * plan->in_dim * plan->C * sizeof(float) + 255) / 256) * 256 + 256;     // per-edge grad_feats rows
     if (plan->bwd_v2 && plan->bwd_nroles > 1) b += (size_t)plan->bwd_nroles * n_edges * plan->sh_dim * sizeof(float) + 256;   // per-role grad_sh
     return b;
+}
+
+static size_t gsh_parts_offset(const e3_plan *plan, int64_t n_edges)
+{
+    return (((size_t)n_edges * plan->in_dim * plan->C * sizeof(float) + 255) / 256) * 256;
+}
+
+// first VJP phase for a receiver range (offset row_ptr / grad_out pointers, absolute edge- and sender-indexed tensors):
+// grad_weights, per-edge grad_feats rows (workspace) and grad_sh (per-role partial buffers when the plan has several roles)
+static int launch_bwd_phase1(const e3_plan *plan, const void *feats, const void *sh, const void *weights, const int32_t *senders,
+                             const int32_t *row_ptr, int32_t n_nodes, const float *grad_out, float *grad_sh, void *grad_weights,
+                             void *workspace, int64_t n_edges_total, cudaStream_t st, int32_t heur_nodes = -1)
+{
+    if (n_nodes == 0 || n_edges_total == 0) return E3_OK;
+    if (heur_nodes < 1) heur_nodes = n_nodes;
+    if (!plan->bwd.fn) { set_error("plan has no loaded backward kernel"); return E3_ERR_CUDA; }
+    float *dxe = (float *)workspace;
+    const int roles = plan->bwd_v2 ? plan->bwd_nroles : 1;
+    // one CTA per (receiver, role, part); its warps split the receiver's edges.  Small graphs are cut into `split`
+    // parts per receiver so that the grid still covers the machine several times over (tail effect).
+    int split = 1;
+    if (plan->bwd_v2) {
+        split = plan->bwd_split;
+        if (split <= 0) {
+            const long long slots = (long long)plan->n_sm * plan->bwd_ctas_per_sm;
+            split = (int)((8 * slots + heur_nodes - 1) / heur_nodes);
+            split = split < 1 ? 1 : (split > 4 ? 4 : split);
+        }
+    }
+    long long grid = (long long)n_nodes * split;
+    if (plan->bwd_v2) {           // CTA order: chunk of receivers, then role, then (receiver, part)
+        const long long chunks = ((long long)n_nodes + plan->bwd_chunk - 1) / plan->bwd_chunk;
+        grid = chunks * plan->bwd_chunk * plan->bwd_nroles * split;
+    }
+    if (grid > 0x7fffffffLL) { set_error("grid too large"); return E3_ERR_UNSUPPORTED; }
+    float *gsh_arg = roles > 1 ? reinterpret_cast<float *>(reinterpret_cast<char *>(workspace) + gsh_parts_offset(plan, n_edges_total)) : grad_sh;
+    long long ne = n_edges_total;
+    void *args[] = { (void *)&feats, (void *)&sh, (void *)&weights, (void *)&senders, (void *)&row_ptr, (void *)&grad_out,
+                     (void *)&dxe, (void *)&gsh_arg, (void *)&grad_weights, (void *)&n_nodes, (void *)&split, (void *)&ne };
+    E3_CUDA_TRY(cudaLaunchKernel((const void *)plan->bwd.fn, dim3((unsigned)grid), dim3(plan->bwd.threads), args, plan->bwd.smem_dyn, st));
+    return E3_OK;
+}
+
+// second VJP phase: per-sender sum of the workspace rows, sum of the per-role grad_sh buffers
+static int launch_bwd_phase2(const e3_plan *plan, const int32_t *perm_s, const int32_t *col_ptr, int64_t n_edges, int32_t n_nodes,
+                             float *grad_feats, float *grad_sh, void *workspace, cudaStream_t st)
+{
+    const int roles = plan->bwd_v2 ? plan->bwd_nroles : 1;
+    int rc = launch_dx_reduce((const float *)workspace, perm_s, col_ptr, n_nodes, plan->in_dim * plan->C, grad_feats, st);
+    if (rc == E3_OK && roles > 1 && n_edges > 0)
+        rc = launch_gsh_reduce(reinterpret_cast<const float *>(reinterpret_cast<const char *>(workspace) + gsh_parts_offset(plan, n_edges)),
+                               roles, n_edges * plan->sh_dim, grad_sh, st);
+    return rc;
 }
 
 extern "C" int e3_tp_scatter_bwd(const e3_plan *plan, const void *feats, const void *sh, const void *weights,
@@ -270,42 +332,10 @@ extern "C" int e3_tp_scatter_bwd(const e3_plan *plan, const void *feats, const v
         return E3_ERR_WORKSPACE;
     }
     if (n_nodes == 0) return E3_OK;
-    if (!plan->bwd.fn) { set_error("plan has no loaded backward kernel"); return E3_ERR_CUDA; }
-    float *dxe = (float *)workspace;
-    float *gsh_parts = nullptr;
-    const int roles = plan->bwd_v2 ? plan->bwd_nroles : 1;
-    if (n_edges > 0) {
-        // one CTA per (receiver, part); its warps split the receiver's edges.  Small graphs are cut into `split`
-        // parts per receiver so that the grid still covers the machine several times over (tail effect).
-        int split = 1;
-        if (plan->bwd_v2) {
-            split = plan->bwd_split;
-            if (split <= 0) {
-                const long long slots = (long long)plan->n_sm * plan->bwd_ctas_per_sm;
-                split = (int)((8 * slots + n_nodes - 1) / n_nodes);
-                split = split < 1 ? 1 : (split > 4 ? 4 : split);
-            }
-        }
-        long long grid = (long long)n_nodes * split;
-        if (plan->bwd_v2) {           // CTA order: chunk of receivers, then role, then (receiver, part)
-            const long long chunks = ((long long)n_nodes + plan->bwd_chunk - 1) / plan->bwd_chunk;
-            grid = chunks * plan->bwd_chunk * plan->bwd_nroles * split;
-        }
-        if (grid > 0x7fffffffLL) { set_error("grid too large"); return E3_ERR_UNSUPPORTED; }
-        if (roles > 1) {
-            const size_t off = (((size_t)n_edges * plan->in_dim * plan->C * sizeof(float) + 255) / 256) * 256;
-            gsh_parts = reinterpret_cast<float *>(reinterpret_cast<char *>(workspace) + off);
-        }
-        float *gsh_arg = roles > 1 ? gsh_parts : grad_sh;
-        long long ne = n_edges;
-        void *args[] = { (void *)&feats, (void *)&sh, (void *)&weights, (void *)&senders, (void *)&row_ptr, (void *)&grad_out,
-                         (void *)&dxe, (void *)&gsh_arg, (void *)&grad_weights, (void *)&n_nodes, (void *)&split, (void *)&ne };
-        E3_CUDA_TRY(cudaLaunchKernel((const void *)plan->bwd.fn, dim3((unsigned)grid), dim3(plan->bwd.threads), args, plan->bwd.smem_dyn, S(stream)));
-    }
+    int rc = launch_bwd_phase1(plan, feats, sh, weights, senders, row_ptr, n_nodes, grad_out, grad_sh, grad_weights, workspace, n_edges, S(stream));
+    if (rc != E3_OK) return rc;
     if (plan->mid_event) E3_CUDA_TRY(cudaEventRecord(plan->mid_event, S(stream)));
-    int rc = launch_dx_reduce(dxe, perm_s, col_ptr, n_nodes, plan->in_dim * plan->C, grad_feats, S(stream));
-    if (rc == E3_OK && roles > 1 && n_edges > 0) rc = launch_gsh_reduce(gsh_parts, roles, n_edges * plan->sh_dim, grad_sh, S(stream));
-    return rc;
+    return launch_bwd_phase2(plan, perm_s, col_ptr, n_edges, n_nodes, grad_feats, grad_sh, workspace, S(stream));
 }
 
 extern "C" int e3_profile_set_mid_event(e3_plan *plan, void *cuda_event)
@@ -315,14 +345,24 @@ extern "C" int e3_profile_set_mid_event(e3_plan *plan, void *cuda_event)
     return E3_OK;
 }
 
+extern "C" int e3_measure_fp32_peak(double *tflops, double ms_target, e3_stream stream)
+{
+    if (!tflops || !(ms_target > 0.0)) { set_error("e3_measure_fp32_peak: bad arguments"); return E3_ERR_INVALID_ARG; }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); set_error("no CUDA device"); return E3_ERR_CUDA; }
+    return measure_fp32_peak(tflops, ms_target, S(stream));
+}
+
 // ---------------------------------------------------------------------------------------------
 // host-buffer session
 // ---------------------------------------------------------------------------------------------
 struct e3_session {
+    static constexpr int kMaxChunks = 64;
     const e3_plan *plan = nullptr;
     int64_t max_edges = 0;
     int32_t max_nodes = 0;
-    cudaStream_t stream = nullptr;
+    cudaStream_t stream = nullptr, stream_in = nullptr, stream_out = nullptr;
+    cudaEvent_t ev_small = nullptr, ev_done = nullptr, ev_in[kMaxChunks] = {}, ev_fwd[kMaxChunks] = {}, ev_bwd[kMaxChunks] = {};
     float *vec = nullptr, *out = nullptr, *gout = nullptr, *gfeats = nullptr, *gsh = nullptr, *gvec = nullptr, *forces = nullptr;
     void *feats = nullptr, *sh = nullptr, *weights = nullptr, *gweights = nullptr, *ws = nullptr, *gws = nullptr;
     int32_t *snd = nullptr, *rcv = nullptr, *row_ptr = nullptr, *perm_s = nullptr, *col_ptr = nullptr;
@@ -335,7 +375,16 @@ extern "C" int e3_session_destroy(e3_session *s)
     void *ptrs[] = { s->vec, s->out, s->gout, s->gfeats, s->gsh, s->gvec, s->forces, s->feats, s->sh, s->weights, s->gweights,
                      s->ws, s->gws, s->snd, s->rcv, s->row_ptr, s->perm_s, s->col_ptr };
     for (void *p : ptrs) if (p) cudaFree(p);
+    for (int k = 0; k < e3_session::kMaxChunks; ++k) {
+        if (s->ev_in[k]) cudaEventDestroy(s->ev_in[k]);
+        if (s->ev_fwd[k]) cudaEventDestroy(s->ev_fwd[k]);
+        if (s->ev_bwd[k]) cudaEventDestroy(s->ev_bwd[k]);
+    }
+    if (s->ev_small) cudaEventDestroy(s->ev_small);
+    if (s->ev_done) cudaEventDestroy(s->ev_done);
     if (s->stream) cudaStreamDestroy(s->stream);
+    if (s->stream_in) cudaStreamDestroy(s->stream_in);
+    if (s->stream_out) cudaStreamDestroy(s->stream_out);
     delete s;
     return E3_OK;
 }
@@ -352,6 +401,15 @@ extern "C" int e3_session_create(e3_session **session, const e3_plan *plan, int6
     s->ws_bytes = e3_bwd_workspace_bytes(plan, max_edges, max_nodes);
     s->gws_bytes = graph_workspace_bytes(max_edges, max_nodes);
     cudaError_t e = cudaStreamCreateWithFlags(&s->stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s->stream_in, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s->stream_out, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&s->ev_small, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&s->ev_done, cudaEventDisableTiming);
+    for (int k = 0; k < e3_session::kMaxChunks && e == cudaSuccess; ++k) {
+        e = cudaEventCreateWithFlags(&s->ev_in[k], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&s->ev_fwd[k], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&s->ev_bwd[k], cudaEventDisableTiming);
+    }
 #define SALLOC(ptr, bytes) if (e == cudaSuccess) e = cudaMalloc((void **)&(ptr), (bytes))
     SALLOC(s->vec, E * 3 * 4); SALLOC(s->gvec, E * 3 * 4); SALLOC(s->forces, N * 3 * 4);
     SALLOC(s->feats, N * plan->in_dim * C * es); SALLOC(s->gfeats, N * plan->in_dim * C * 4);
@@ -366,6 +424,11 @@ extern "C" int e3_session_create(e3_session **session, const e3_plan *plan, int6
     return E3_OK;
 }
 
+// The run is pipelined over contiguous receiver ranges ("chunks"): the weights of chunk k+1 travel host->device on one
+// copy stream while chunk k is computed, and chunk k-1's `out` rows and grad_weights travel device->host on another
+// (PCIe is full duplex; the weights and their gradients are > 95 % of the bytes).  Results do not depend on the chunking:
+// a chunk is the same kernels, in the launch shape chosen for the whole graph, on a receiver range, and the per-sender
+// reduction runs once at the end.
 extern "C" int e3_session_run_host(e3_session *s, const float *vec_h, const void *feats_h, const void *weights_h,
                                    const int32_t *senders_h, const int32_t *receivers_h, int64_t n_edges, int32_t n_nodes,
                                    const float *grad_out_h, float *out_h, float *grad_feats_h, void *grad_weights_h,
@@ -378,32 +441,73 @@ extern "C" int e3_session_run_host(e3_session *s, const float *vec_h, const void
     }
     const e3_plan *pl = s->plan;
     const size_t E = (size_t)n_edges, N = (size_t)n_nodes, es = esize(pl), P = pl->paths.size(), C = pl->C;
-    cudaStream_t st = s->stream;
+    const size_t in_row = (size_t)pl->in_dim * C, out_row = (size_t)pl->out_dim * C, w_row = P * C;
+    cudaStream_t st = s->stream, sin = s->stream_in, sout = s->stream_out;
     int64_t up = 0, down = 0;
-#define H2D(dst, src, bytes) do { if ((bytes) > 0) { E3_CUDA_TRY(cudaMemcpyAsync((dst), (src), (bytes), cudaMemcpyHostToDevice, st)); up += (int64_t)(bytes); } } while (0)
-#define D2H(dst, src, bytes) do { if ((dst) && (bytes) > 0) { E3_CUDA_TRY(cudaMemcpyAsync((dst), (src), (bytes), cudaMemcpyDeviceToHost, st)); down += (int64_t)(bytes); } } while (0)
-    H2D(s->snd, senders_h, E * 4); H2D(s->rcv, receivers_h, E * 4); H2D(s->vec, vec_h, E * 12);
-    H2D(s->feats, feats_h, N * pl->in_dim * C * es); H2D(s->weights, weights_h, E * P * C * es);
+#define H2D(stream_, dst, src, bytes) do { if ((bytes) > 0) { E3_CUDA_TRY(cudaMemcpyAsync((dst), (src), (bytes), cudaMemcpyHostToDevice, (stream_))); up += (int64_t)(bytes); } } while (0)
+#define D2H(stream_, dst, src, bytes) do { if ((dst) && (bytes) > 0) { E3_CUDA_TRY(cudaMemcpyAsync((dst), (src), (bytes), cudaMemcpyDeviceToHost, (stream_))); down += (int64_t)(bytes); } } while (0)
+    // small inputs first
+    H2D(sin, s->snd, senders_h, E * 4); H2D(sin, s->rcv, receivers_h, E * 4); H2D(sin, s->vec, vec_h, E * 12);
+    H2D(sin, s->feats, feats_h, N * in_row * es);
+    if (grad_out_h) H2D(sin, s->gout, grad_out_h, N * out_row * 4);
+    E3_CUDA_TRY(cudaEventRecord(s->ev_small, sin));
+    E3_CUDA_TRY(cudaStreamWaitEvent(st, s->ev_small, 0));
     int rc = launch_graph_prepare(s->snd, s->rcv, n_edges, n_nodes, s->row_ptr, s->perm_s, s->col_ptr, s->gws, s->gws_bytes, 0, st);
     if (rc == E3_OK) rc = e3_sh_fwd(pl, s->vec, n_edges, s->sh, st);
-    if (rc == E3_OK) rc = e3_tp_scatter_fwd(pl, s->feats, s->sh, s->weights, s->snd, s->rcv, s->row_ptr, n_edges, n_nodes, s->out, st);
     if (rc != E3_OK) return rc;
-    D2H(out_h, s->out, N * pl->out_dim * C * 4);
+    // receiver ranges of roughly equal edge counts (~48 MB of weights each); rows must stay 16-byte aligned under the offsets
+    int n_chunks = (int)((E * w_row * es + (48u << 20) - 1) / (48u << 20));
+    n_chunks = n_chunks < 1 ? 1 : (n_chunks > e3_session::kMaxChunks ? e3_session::kMaxChunks : n_chunks);
+    if ((out_row * 4) % 16 != 0 || (w_row * es) % 16 != 0 || n_nodes == 0) n_chunks = 1;
+    int32_t r_lo = 0;
+    int n_used = 0;
+    for (int k = 0; k < n_chunks && r_lo < n_nodes; ++k) {
+        int32_t r_hi = n_nodes;
+        if (k + 1 < n_chunks && n_edges > 0) {
+            const int64_t e_target = (int64_t)((double)(k + 1) / n_chunks * (double)n_edges);
+            r_hi = e_target < n_edges ? receivers_h[e_target] : n_nodes;      // receivers_h is sorted: edges of r < r_hi come first
+            if (r_hi <= r_lo) continue;
+        }
+        // edges of receivers [r_lo, r_hi): [e_lo, e_hi) by binary search in the sorted host array
+        auto lower = [&](int32_t r) { int64_t a = 0, b = n_edges; while (a < b) { int64_t m = (a + b) / 2; if (receivers_h[m] < r) a = m + 1; else b = m; } return a; };
+        const int64_t e_lo = lower(r_lo), e_hi = lower(r_hi);
+        const int32_t nr = r_hi - r_lo;
+        H2D(sin, (char *)s->weights + (size_t)e_lo * w_row * es, (const char *)weights_h + (size_t)e_lo * w_row * es, (size_t)(e_hi - e_lo) * w_row * es);
+        E3_CUDA_TRY(cudaEventRecord(s->ev_in[n_used], sin));
+        E3_CUDA_TRY(cudaStreamWaitEvent(st, s->ev_in[n_used], 0));
+        rc = launch_fwd(pl, s->feats, s->sh, s->weights, s->snd, s->row_ptr + r_lo, nr, s->out + (size_t)r_lo * out_row, st, n_nodes);
+        if (rc != E3_OK) return rc;
+        E3_CUDA_TRY(cudaEventRecord(s->ev_fwd[n_used], st));
+        E3_CUDA_TRY(cudaStreamWaitEvent(sout, s->ev_fwd[n_used], 0));
+        D2H(sout, out_h ? out_h + (size_t)r_lo * out_row : nullptr, s->out + (size_t)r_lo * out_row, (size_t)nr * out_row * 4);
+        if (grad_out_h) {
+            rc = launch_bwd_phase1(pl, s->feats, s->sh, s->weights, s->snd, s->row_ptr + r_lo, nr, s->gout + (size_t)r_lo * out_row, s->gsh,
+                                   grad_weights_h ? s->gweights : nullptr, s->ws, n_edges, st, n_nodes);
+            if (rc != E3_OK) return rc;
+            E3_CUDA_TRY(cudaEventRecord(s->ev_bwd[n_used], st));
+            E3_CUDA_TRY(cudaStreamWaitEvent(sout, s->ev_bwd[n_used], 0));
+            D2H(sout, grad_weights_h ? (char *)grad_weights_h + (size_t)e_lo * w_row * es : nullptr, (char *)s->gweights + (size_t)e_lo * w_row * es,
+                (size_t)(e_hi - e_lo) * w_row * es);
+        }
+        r_lo = r_hi;
+        ++n_used;
+    }
     if (grad_out_h) {
-        H2D(s->gout, grad_out_h, N * pl->out_dim * C * 4);
-        rc = e3_tp_scatter_bwd(pl, s->feats, s->sh, s->weights, s->snd, s->rcv, s->row_ptr, s->perm_s, s->col_ptr, n_edges, n_nodes,
-                               s->gout, s->gfeats, s->gsh, grad_weights_h ? s->gweights : nullptr, s->ws, s->ws_bytes, st);
+        rc = launch_bwd_phase2(pl, s->perm_s, s->col_ptr, n_edges, n_nodes, s->gfeats, s->gsh, s->ws, st);
         if (rc == E3_OK) rc = e3_sh_bwd(pl, s->vec, s->gsh, n_edges, s->gvec, st);
         if (rc == E3_OK && forces_h) rc = e3_force_reduce(s->gvec, s->row_ptr, s->perm_s, s->col_ptr, n_edges, n_nodes, s->forces, st);
         if (rc != E3_OK) return rc;
-        D2H(grad_feats_h, s->gfeats, N * pl->in_dim * C * 4);
-        D2H(grad_weights_h, s->gweights, E * P * C * es);
-        D2H(grad_vec_h, s->gvec, E * 12);
-        D2H(forces_h, s->forces, N * 12);
+        E3_CUDA_TRY(cudaEventRecord(s->ev_done, st));
+        E3_CUDA_TRY(cudaStreamWaitEvent(sout, s->ev_done, 0));
+        D2H(sout, grad_feats_h, s->gfeats, N * in_row * 4);
+        D2H(sout, grad_vec_h, s->gvec, E * 12);
+        D2H(sout, forces_h, s->forces, N * 12);
     }
 #undef H2D
 #undef D2H
+    E3_CUDA_TRY(cudaStreamSynchronize(sin));
     E3_CUDA_TRY(cudaStreamSynchronize(st));
+    E3_CUDA_TRY(cudaStreamSynchronize(sout));
     if (bytes_h2d) *bytes_h2d = up;
     if (bytes_d2h) *bytes_d2h = down;
     return E3_OK;

@@ -122,6 +122,7 @@ int launch_force_reduce(const float *gvec, const int32_t *row_ptr, const int32_t
 int launch_dx_reduce(const float *dxe, const int32_t *perm_s, const int32_t *col_ptr, int32_t N, int row_len,
                      float *dx, cudaStream_t st);
 int launch_gsh_reduce(const float *parts, int n_parts, int64_t n, float *gsh, cudaStream_t st);
+int measure_fp32_peak(double *tflops, double ms_target, cudaStream_t st);
 int launch_cg_planner(const int *triples /*[n,3] host*/, int n, std::vector<std::vector<double>> &dense_out);
 
 }  // namespace e3

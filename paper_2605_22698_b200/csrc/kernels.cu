@@ -397,4 +397,54 @@ int launch_dx_reduce(const float *dxe, const int32_t *perm_s, const int32_t *col
     return E3_OK;
 }
 
+// ---------------------------------------------------------------------------------------------
+// FP32 ceiling of this board: register-only packed FMAs (e3_measure_fp32_peak)
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(1024, 2) ffma_peak_kernel(float *sink, int iters, float a, float b)
+{
+    float2 c0 = make_float2(threadIdx.x, 1.f), c1 = make_float2(2.f, 3.f), c2 = make_float2(4.f, 5.f), c3 = make_float2(6.f, 7.f);
+    float2 c4 = make_float2(8.f, 9.f), c5 = make_float2(10.f, 11.f), c6 = make_float2(12.f, 13.f), c7 = make_float2(14.f, 15.f);
+    const float2 x = make_float2(a, a), y = make_float2(b, b);
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            c0 = __ffma2_rn(c0, x, y); c1 = __ffma2_rn(c1, x, y); c2 = __ffma2_rn(c2, x, y); c3 = __ffma2_rn(c3, x, y);
+            c4 = __ffma2_rn(c4, x, y); c5 = __ffma2_rn(c5, x, y); c6 = __ffma2_rn(c6, x, y); c7 = __ffma2_rn(c7, x, y);
+        }
+    }
+    const float r = c0.x + c0.y + c1.x + c1.y + c2.x + c2.y + c3.x + c3.y + c4.x + c4.y + c5.x + c5.y + c6.x + c6.y + c7.x + c7.y;
+    if (r == 12345.678f) sink[0] = r;      // never true for the arguments used; keeps the chains alive
+}
+
+int measure_fp32_peak(double *tflops, double ms_target, cudaStream_t st)
+{
+    int dev = 0, nsm = 0;
+    E3_CUDA_TRY(cudaGetDevice(&dev));
+    E3_CUDA_TRY(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    float *sink = nullptr;
+    E3_CUDA_TRY(cudaMalloc(&sink, 16));
+    cudaEvent_t e0, e1;
+    E3_CUDA_TRY(cudaEventCreate(&e0));
+    E3_CUDA_TRY(cudaEventCreate(&e1));
+    const int grid = nsm * 2;
+    const double flop_per_iter = (double)grid * 1024 * 16 * 8 * 2 * 2;      // 16 x 8 FFMA2 = 2 lanes x 2 flop each
+    int iters = 2000;
+    float ms = 0.f;
+    for (int pass = 0; pass < 2; ++pass) {           // pass 0 calibrates (and warms up), pass 1 runs for ~ms_target
+        cudaEventRecord(e0, st);
+        ffma_peak_kernel<<<grid, 1024, 0, st>>>(sink, iters, 0.999f, 0.001f);
+        cudaEventRecord(e1, st);
+        cudaError_t e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) { cudaFree(sink); return cuda_fail(e, "ffma_peak_kernel"); }
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (pass == 0 && ms > 0.f) {
+            double want = (double)iters * ms_target / ms;
+            iters = want > 2e9 ? 2000000000 : (want < 100 ? 100 : (int)want);
+        }
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+    if (tflops) *tflops = flop_per_iter * iters / (ms * 1e-3) / 1e12;
+    return E3_OK;
+}
+
 }  // namespace e3

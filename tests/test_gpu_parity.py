@@ -287,3 +287,26 @@ def test_session_host_path_matches_device_path():
     assert down == sum(t.numel() * 4 for t in (out, dx, dw, dvec, F))
     for name, t in (("out", out), ("dx", dx), ("dw", dw), ("dvec", dvec), ("F", F)):
         assert np.array_equal(t.numpy(), dev[name]), name
+
+
+def test_session_pipelined_chunks_match_device_path():
+    """154 MB of weights => the host path runs in 4 receiver-range chunks on three streams; every result must be
+    bit-identical to the unchunked device entry points (and hence within the oracle bars checked elsewhere)."""
+    cfg = W.small_config(n_atoms=1536, channels=32, irreps_in=((0, 1), (1, -1), (2, 1)), sh_lmax=2, out_lmax=2,
+                         box=24.8579, k=107)
+    pl, g, x, w, G = make_case(cfg)
+    assert w.nbytes > 3 * (48 << 20)
+    plan = gpu_plan(pl)
+    dev = run_gpu(plan, g, x, w, G)
+    s = B.Session(plan, g.n_edges, g.n_nodes)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    out = torch.empty((g.n_nodes, plan.out_dim * plan.channels)).pin_memory()
+    dx = torch.empty((g.n_nodes, plan.in_dim * plan.channels)).pin_memory()
+    dw = torch.empty((g.n_edges, plan.weights_per_edge)).pin_memory()
+    dvec = torch.empty((g.n_edges, 3)).pin_memory()
+    F = torch.empty((g.n_nodes, 3)).pin_memory()
+    for _ in range(2):
+        up, down = s.run_host(pin(g.vec), pin(x), pin(w), pin(g.senders), pin(g.receivers), g.n_nodes, pin(G), out, dx, dw, dvec, F)
+        assert up == g.vec.nbytes + x.nbytes + w.nbytes + 2 * g.senders.nbytes + G.nbytes
+        for name, t in (("out", out), ("dx", dx), ("dw", dw), ("dvec", dvec), ("F", F)):
+            assert np.array_equal(t.numpy(), dev[name]), name
