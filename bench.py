@@ -185,6 +185,20 @@ def run_reference(args):
 # --------------------------------------------------------------------------------------------
 # our arm
 # --------------------------------------------------------------------------------------------
+def aggregate_replicas(elapsed_ms, n_edges, steps, world, device):
+    """Replicas-only multi-GPU aggregation: every rank runs the same workload on its own GPU with
+    no data-path collective; the job time is the MAX of the ranks' device times and `value` the edges ALL ranks
+    processed divided by it.  Returns (elapsed_ms over ranks, whole-job edges/s).  The only collective is this
+    one-element all-reduce (NCCL on GPUs; the CPU tests run it over gloo)."""
+    if world > 1:
+        import torch
+        import torch.distributed as dist
+        t = torch.tensor([elapsed_ms], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        elapsed_ms = float(t.item())
+    return elapsed_ms, world * n_edges * steps / (elapsed_ms * 1e-3)
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -293,12 +307,7 @@ def run_ours(args):
     t_stop.record(stream)
     barrier()
     clocks = sampler.stop()
-    elapsed_ms = t_start.elapsed_time(t_stop)
-    if world > 1:
-        t = torch.tensor([elapsed_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        elapsed_ms = float(t.item())
-    value = world * E * args.steps / (elapsed_ms * 1e-3)
+    elapsed_ms, value = aggregate_replicas(t_start.elapsed_time(t_stop), E, args.steps, world, dev)
 
     # per-call / per-kernel device times, measured live with events on the launching stream over
     # a second pass of the same steps (events between calls would otherwise perturb `value`)
