@@ -113,7 +113,7 @@ def _tiny(rng, n, e):
     return snd[o].astype(np.int32), rcv[o].astype(np.int32)
 
 
-@pytest.mark.parametrize("C", [1, 3, 4, 32, 33, 64, 96, 128])
+@pytest.mark.parametrize("C", [1, 3, 4, 8, 16, 32, 33, 64, 96, 128, 256])
 def test_channel_counts_and_ragged_lanes(C):
     rng = np.random.default_rng(C)
     cfg = W.small_config(n_atoms=9, channels=C, irreps_in=((0, 1), (1, -1), (2, 1)), sh_lmax=2, out_lmax=2)
@@ -256,6 +256,30 @@ def test_bf16_storage_parity_and_fp32_recovers():
     e32 = compare(run_gpu(plan32, g, x, w, G), run_oracle(pl, g, x, w, G))
     assert e32["out"] < 1e-5 and e32["dw"] < 1e-4
     print("bf16", errs, "f32", e32)
+
+
+@pytest.mark.parametrize("C,lmax", [(32, 3), (64, 3), (256, 3), (64, 2)])
+def test_bf16_storage_channel_counts(C, lmax):
+    """bf16 storage with 4 / 2 edges per warp step, two 128-channel blocks per edge (C = 256: grad_sh accumulates over the
+    blocks), and lmax = 2 (odd SH row: the first-generation direct-load kernels)."""
+    rng = np.random.default_rng(300 + C + lmax)
+    irr = ((0, 1), (1, -1), (2, 1), (3, -1))[: lmax + 1]
+    cfg = W.small_config(channels=C, irreps_in=irr, sh_lmax=lmax, out_lmax=lmax, storage="bf16")
+    pl = plan_inputs(cfg)
+    n = 17
+    deg = rng.integers(0, 9, size=n); deg[3] = 41
+    rcv = np.repeat(np.arange(n), deg)
+    snd = rng.integers(0, n, size=rcv.size)
+    o = np.lexsort((snd, rcv))
+    snd, rcv = snd[o].astype(np.int32), rcv[o].astype(np.int32)
+    e = rcv.size
+    in_dim, out_dim = sum(2 * l + 1 for l, _ in irr), sum(2 * l + 1 for l, _, _ in pl[2])
+    g = W.Graph(n, np.zeros((n, 3)), snd, rcv, (rng.normal(size=(e, 3)) * 2).astype(np.float32), 0.0)
+    x = W.round_to_storage(rng.normal(size=(n, in_dim * C)), "bf16")
+    w = W.round_to_storage(rng.normal(size=(e, len(pl[3]) * C)), "bf16")
+    G = rng.normal(size=(n, out_dim * C)).astype(np.float32)
+    plan = gpu_plan(pl, "bf16")
+    compare(run_gpu(plan, g, x, w, G), run_oracle(pl, g, x, w, G, storage="bf16"), tol_fwd=TOL_BF16, tol_vjp=TOL_BF16, tol_sh=8e-3)
 
 
 # ------------------------------------------------------------------ determinism
