@@ -73,7 +73,7 @@ struct e3_plan {
     int nchb2 = 1;             // v2: channel blocks of 128
     int fwd_depth = 4;         // forward ring stages (power of two); the backward ring has one rolling stage
     int fwd_depth_max = 6;     // v2 forward: roles with small stages deepen their ring up to this many stages
-    int fwd_chunk = 512;       // CTAs per (chunk, role): CTA order is chunk-major, then role
+    int fwd_chunk = 16;        // CTAs per (chunk, role): CTA order is chunk-major, then role
     int fwd_minb = 4, bwd_minb = 2;        // __launch_bounds__ min blocks per SM
     int bwd_v2 = 0;            // 1: second-generation backward (codegen2.cpp)
     int bwd_r = 0;             // v2 backward: weights ring holds 1/bwd_r of a unit (0 = choose; set by the generator)
