@@ -32,7 +32,7 @@ FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # nominal FFMA peak (DESI
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the ncu --set full
 # capture named in profiles/ (filled in per round; None when no capture exists for that workload)
 NCU_TRAFFIC_BYTES = {
-    "cfg2_mace_1536atoms_128ch_l3": 1253263872,     # profiles/r01b_cfg2_full.md: e3_bwd 595.66 MB read + 657.60 MB written
+    "cfg2_mace_1536atoms_128ch_l3": 1251569920,     # profiles/r01c_cfg2_full.md: e3_bwd 595.83 MB read + 655.74 MB written
     "cfg4_100k_64ch_l3": 119887406000,              # profiles/r01b_cfg4_full.md: e3_bwd 51.93 GB read + 67.96 GB written
 }
 
