@@ -334,3 +334,9 @@ def test_session_pipelined_chunks_match_device_path():
         assert up == g.vec.nbytes + x.nbytes + w.nbytes + 2 * g.senders.nbytes + G.nbytes
         for name, t in (("out", out), ("dx", dx), ("dw", dw), ("dvec", dvec), ("F", F)):
             assert np.array_equal(t.numpy(), dev[name]), name
+
+
+def test_fp32_peak_measurement_aid():
+    """e3_measure_fp32_peak (bench.py's `alu_peak.measured_sustained_tflops`): a sane fraction of 148 x 128 x 2 x 1.965 GHz."""
+    t = B.e3_measure_fp32_peak(30.0)
+    assert 0.4 * 74.45 < t < 1.05 * 74.45, t
