@@ -76,6 +76,8 @@ int e3_all_paths(const e3_irrep *irreps_in, int n_in, int sh_lmax, int out_lmax,
  * forward and VJP kernels for this plan (coefficients become FFMA immediates).  Needs a device;
  * synchronises; takes O(seconds) once.  A path whose i_out is shared with another path ADDS
  * into that block (A6).  Limits: l <= 3 everywhere, all multiplicities equal.
+ * Environment: E3_TUNE="key=value,..." overrides launch-shape heuristics (never results);
+ * E3_JIT_CACHE=0 disables the compiled-kernel cache under /tmp/e3b200_jit (keyed by the generated source; speed only).
  * -------------------------------------------------------------------------------------------*/
 int e3_plan_create(e3_plan **plan, const e3_irrep *irreps_in, int n_in, int sh_lmax,
                    const e3_irrep *irreps_out, int n_out, const e3_path *paths, int n_paths, e3_dtype dtype);

@@ -3,6 +3,7 @@
 // a GPU driver, where it is only ever used for the build check).
 #include <nvrtc.h>
 #include <sys/stat.h>
+#include <unistd.h>
 
 #include <cstdio>
 #include <cstdlib>
@@ -41,6 +42,31 @@ int jit_compile(JitKernel &k, const std::string &file_hint)
     std::string path = file_hint.empty() ? dir + "/" + k.name + "_" + hb + ".cu" : file_hint;
     if (FILE *f = fopen(path.c_str(), "w")) { fwrite(k.source.data(), 1, k.source.size(), f); fclose(f); }
 
+    // compiled-code cache (speed only: the key is the hash of the generated source plus the NVRTC version; E3_JIT_CACHE=0 disables it)
+    int vmaj = 0, vmin = 0;
+    nvrtcVersion(&vmaj, &vmin);
+    char vb[64];
+    snprintf(vb, sizeof(vb), "_%zu_nvrtc%d_%d", k.source.size(), vmaj, vmin);
+    const char *cache_env = getenv("E3_JIT_CACHE");
+    const bool use_cache = !(cache_env && cache_env[0] == '0') && file_hint.empty();
+    const std::string cpath = dir + "/" + k.name + "_" + hb + vb + ".cubin", ipath = cpath + ".info";
+    if (use_cache) {
+        FILE *fi = fopen(ipath.c_str(), "r"), *fc = fopen(cpath.c_str(), "rb");
+        long long want = -1;
+        int regs = 0, spill = 0, smem = 0;
+        if (fi && fc && fscanf(fi, "%lld %d %d %d", &want, &regs, &spill, &smem) == 4 && want > 0) {
+            k.cubin.resize((size_t)want);
+            if (fread(k.cubin.data(), 1, (size_t)want, fc) == (size_t)want && fgetc(fc) == EOF) {
+                fclose(fi); fclose(fc);
+                k.regs = regs; k.spill = spill; k.smem = smem;
+                return E3_OK;
+            }
+            k.cubin.clear();
+        }
+        if (fi) fclose(fi);
+        if (fc) fclose(fc);
+    }
+
     nvrtcProgram prog;
     if (nvrtcCreateProgram(&prog, k.source.c_str(), path.c_str(), 0, nullptr, nullptr) != NVRTC_SUCCESS) {
         set_error("nvrtcCreateProgram failed");
@@ -69,6 +95,18 @@ int jit_compile(JitKernel &k, const std::string &file_hint)
     k.spill = parse_after(log, k.name, "stack frame,", "bytes spill stores");
     int sm = parse_after(log, k.name, ",", "bytes smem");
     k.smem = sm < 0 ? 0 : sm;
+    if (use_cache) {      // write to a temporary name and rename: concurrent processes (one per GPU) may build the same plan
+        char tb[64];
+        snprintf(tb, sizeof(tb), ".tmp%ld", (long)getpid());
+        const std::string tc = cpath + tb, ti = ipath + tb;
+        FILE *fc = fopen(tc.c_str(), "wb"), *fi = fopen(ti.c_str(), "w");
+        bool ok = fc && fi && fwrite(k.cubin.data(), 1, k.cubin.size(), fc) == k.cubin.size() &&
+                  fprintf(fi, "%lld %d %d %d\n", (long long)k.cubin.size(), k.regs, k.spill, k.smem) > 0;
+        if (fc) fclose(fc);
+        if (fi) fclose(fi);
+        if (ok) ok = rename(tc.c_str(), cpath.c_str()) == 0 && rename(ti.c_str(), ipath.c_str()) == 0;
+        if (!ok) { remove(tc.c_str()); remove(ti.c_str()); }
+    }
     if (!file_hint.empty()) {
         std::string cp = file_hint + ".cubin";
         if (FILE *f = fopen(cp.c_str(), "wb")) { fwrite(k.cubin.data(), 1, k.cubin.size(), f); fclose(f); }
