@@ -334,6 +334,14 @@ def test_session_pipelined_chunks_match_device_path():
         assert up == g.vec.nbytes + x.nbytes + w.nbytes + 2 * g.senders.nbytes + G.nbytes
         for name, t in (("out", out), ("dx", dx), ("dw", dw), ("dvec", dvec), ("F", F)):
             assert np.array_equal(t.numpy(), dev[name]), name
+    # forward only (no cotangent), and a VJP whose grad_weights are not requested: fewer copies, same numbers
+    out.zero_()
+    up, down = s.run_host(pin(g.vec), pin(x), pin(w), pin(g.senders), pin(g.receivers), g.n_nodes, None, out)
+    assert down == out.numel() * 4 and np.array_equal(out.numpy(), dev["out"])
+    dx.zero_(); F.zero_()
+    up, down = s.run_host(pin(g.vec), pin(x), pin(w), pin(g.senders), pin(g.receivers), g.n_nodes, pin(G), None, dx, None, None, F)
+    assert down == (dx.numel() + F.numel()) * 4
+    assert np.array_equal(dx.numpy(), dev["dx"]) and np.array_equal(F.numpy(), dev["F"])
 
 
 def test_fp32_peak_measurement_aid():
