@@ -16,8 +16,8 @@ TUNES = ["", "fwd_split=2,bwd_split=2", "fwd_split=4,bwd_split=3", "bwd_depth=1"
          "bwd_role_cost=1000000", "rows=12", "chunk=2,bwd_chunk=3", "fwd_depth_max=2"]
 
 
-def _random_case(rng):
-    C = int(rng.choice([4, 8, 16, 32, 64, 128, 256, 12, 48]))
+def _random_case(rng, medium=False):
+    C = int(rng.choice([32, 64, 128] if medium else [4, 8, 16, 32, 64, 128, 256, 12, 48]))
     lmax_in, sh_lmax, out_lmax = (int(rng.integers(0, 4)) for _ in range(3))
     storage = "bf16" if rng.random() < 0.3 else "f32"
     irr = [(l, (1 if rng.random() < 0.5 else -1)) for l in range(lmax_in + 1) if rng.random() < 0.85] or [(0, 1)]
@@ -43,8 +43,12 @@ def _random_case(rng):
                 new_out.append(io)
         irreps_out, paths = new_out, [(a, b, m[c]) for a, b, c in paths]
     pl = (irreps_in, sh_lmax, irreps_out, paths)
-    n = int(rng.integers(1, 40))
-    deg = rng.integers(0, 14, size=n)
+    if medium:                                                                   # several CTA chunks, fsplit = 1 and > 1
+        n = int(rng.integers(150, 2500))
+        deg = rng.integers(0, int(rng.integers(8, 60)), size=n)
+    else:
+        n = int(rng.integers(1, 40))
+        deg = rng.integers(0, 14, size=n)
     if rng.random() < 0.3:
         deg[rng.integers(0, n)] = int(rng.integers(30, 120))
     rcv = np.repeat(np.arange(n), deg)
@@ -64,12 +68,13 @@ def _random_case(rng):
     return pl, storage, g, x, w, G, str(rng.choice(TUNES))
 
 
-@pytest.mark.parametrize("block", range(4))
+@pytest.mark.parametrize("block", range(5))
 def test_random_plans_against_oracle(block, monkeypatch):
     done = 0
-    for it in range(40):
+    medium = block == 4                  # block 4: graphs of 150-2500 nodes, up to ~60k edges
+    for it in range(24 if medium else 40):
         rng = np.random.default_rng(777000 + 1000 * block + it)
-        case = _random_case(rng)
+        case = _random_case(rng, medium)
         if case is None:
             continue
         pl, storage, g, x, w, G, tune = case
@@ -92,4 +97,26 @@ def test_random_plans_against_oracle(block, monkeypatch):
         for k in gpu:
             assert np.array_equal(gpu[k], again[k]), f"{ctx}: {k} differs between two runs"
         done += 1
-    assert done >= 30
+    assert done >= (18 if medium else 30)
+
+
+def test_forward_partial_sums_fit_the_warp_ring(monkeypatch):
+    """Regression (found by the random soak): with bf16 storage and few paths a ring stage is small, and the per-warp ring must
+    still hold the fsplit partial sums (rows x lanes x 16 B): 10 rows x 32 lanes here against 6 stages of 800 B."""
+    rng = np.random.default_rng(78)
+    C = 128
+    pl = ([(0, 1, C)], 3, [(1, -1, C), (3, -1, C)], [(0, 1, 0), (0, 3, 1)])
+    n = 292
+    deg = rng.integers(0, 13, size=n)
+    rcv = np.repeat(np.arange(n), deg)
+    snd = rng.integers(0, n, size=rcv.size)
+    o = np.lexsort((snd, rcv))
+    snd, rcv = snd[o].astype(np.int32), rcv[o].astype(np.int32)
+    e = rcv.size
+    g = W.Graph(n, np.zeros((n, 3)), snd, rcv, (rng.normal(size=(e, 3)) * 2).astype(np.float32), 0.0)
+    x = W.round_to_storage(rng.normal(size=(n, C)), "bf16")
+    w = W.round_to_storage(rng.normal(size=(e, 2 * C)), "bf16")
+    G = rng.normal(size=(n, 10 * C)).astype(np.float32)
+    monkeypatch.setenv("E3_TUNE", "fwd_split=4,bwd_split=3")
+    plan = gpu_plan(pl, "bf16")
+    compare(run_gpu(plan, g, x, w, G), run_oracle(pl, g, x, w, G, storage="bf16"), tol_fwd=TOL_BF16, tol_vjp=TOL_BF16, tol_sh=8e-3)
