@@ -268,21 +268,21 @@ __global__ void force_reduce_kernel(const float *__restrict__ gvec, const int32_
     int32_t i = (int32_t)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
     if (i >= N) return;
     const int lane = threadIdx.x & 31;
-    float fx = 0.0f, fy = 0.0f, fz = 0.0f;
+    // the two sums are kept apart until the end: equal edge sets (self loops) then cancel exactly
+    float ix = 0.0f, iy = 0.0f, iz = 0.0f, ox = 0.0f, oy = 0.0f, oz = 0.0f;
     for (int32_t e = row_ptr[i] + lane; e < row_ptr[i + 1]; e += 32) {
-        fx -= gvec[3 * (int64_t)e]; fy -= gvec[3 * (int64_t)e + 1]; fz -= gvec[3 * (int64_t)e + 2];
+        ix += gvec[3 * (int64_t)e]; iy += gvec[3 * (int64_t)e + 1]; iz += gvec[3 * (int64_t)e + 2];
     }
     for (int32_t j = col_ptr[i] + lane; j < col_ptr[i + 1]; j += 32) {
         int64_t e = perm_s[j];
-        fx += gvec[3 * e]; fy += gvec[3 * e + 1]; fz += gvec[3 * e + 2];
+        ox += gvec[3 * e]; oy += gvec[3 * e + 1]; oz += gvec[3 * e + 2];
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
-        fx += __shfl_xor_sync(0xffffffffu, fx, o);
-        fy += __shfl_xor_sync(0xffffffffu, fy, o);
-        fz += __shfl_xor_sync(0xffffffffu, fz, o);
+        ix += __shfl_xor_sync(0xffffffffu, ix, o); iy += __shfl_xor_sync(0xffffffffu, iy, o); iz += __shfl_xor_sync(0xffffffffu, iz, o);
+        ox += __shfl_xor_sync(0xffffffffu, ox, o); oy += __shfl_xor_sync(0xffffffffu, oy, o); oz += __shfl_xor_sync(0xffffffffu, oz, o);
     }
-    if (lane == 0) { forces[3 * (int64_t)i] = fx; forces[3 * (int64_t)i + 1] = fy; forces[3 * (int64_t)i + 2] = fz; }
+    if (lane == 0) { forces[3 * (int64_t)i] = ox - ix; forces[3 * (int64_t)i + 1] = oy - iy; forces[3 * (int64_t)i + 2] = oz - iz; }
 }
 
 int launch_force_reduce(const float *gvec, const int32_t *row_ptr, const int32_t *perm_s, const int32_t *col_ptr,
