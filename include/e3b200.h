@@ -77,7 +77,10 @@ int e3_all_paths(const e3_irrep *irreps_in, int n_in, int sh_lmax, int out_lmax,
  * synchronises; takes O(seconds) once.  A path whose i_out is shared with another path ADDS
  * into that block (A6).  Limits: l <= 3 everywhere, all multiplicities equal.
  * Environment: E3_TUNE="key=value,..." overrides launch-shape heuristics (never results);
- * E3_JIT_CACHE=0 disables the compiled-kernel cache under /tmp/e3b200_jit (keyed by the generated source; speed only).
+ * E3_JIT_CACHE=0 disables the compiled-kernel cache (speed only).  The cache lives in a per-user directory of mode 0700
+ * ($E3_JIT_DIR, else $XDG_CACHE_HOME/e3b200_jit, else /tmp/e3b200_jit_<uid>; refused if not owned by the caller or
+ * group/world-writable); a hit must match two 64-bit hashes of (compile options + source), the stored source byte for
+ * byte, and the cubin's recorded length and checksum.
  * -------------------------------------------------------------------------------------------*/
 int e3_plan_create(e3_plan **plan, const e3_irrep *irreps_in, int n_in, int sh_lmax,
                    const e3_irrep *irreps_out, int n_out, const e3_path *paths, int n_paths, e3_dtype dtype);
@@ -188,6 +191,9 @@ int e3_force_reduce(const float *grad_vec /*[E,3]*/, const int32_t *row_ptr, con
  * entry points on the same inputs.  Host buffers should be pinned for the overlap.  Any output pointer
  * may be NULL (skipped, and its copy is not made).  Inputs have the plan's storage dtype where
  * the device entry points do.  bytes_h2d / bytes_d2h (may be NULL) receive the bytes copied.
+ * Preconditions, CHECKED on the host before anything is launched (one O(E) pass): every sender / receiver index lies
+ * in [0, n_nodes) (else E3_ERR_INVALID_ARG) and receivers_h is ascending (else E3_ERR_UNSORTED).  On any failing
+ * return the session's three streams have been synchronised: no copy still touches the caller's buffers.
  * -------------------------------------------------------------------------------------------*/
 int e3_session_create(e3_session **session, const e3_plan *plan, int64_t max_edges, int32_t max_nodes);
 int e3_session_destroy(e3_session *session);

@@ -429,7 +429,7 @@ extern "C" int e3_session_create(e3_session **session, const e3_plan *plan, int6
 // (PCIe is full duplex; the weights and their gradients are > 95 % of the bytes).  Results do not depend on the chunking:
 // a chunk is the same kernels, in the launch shape chosen for the whole graph, on a receiver range, and the per-sender
 // reduction runs once at the end.
-extern "C" int e3_session_run_host(e3_session *s, const float *vec_h, const void *feats_h, const void *weights_h,
+static int session_run_host_impl(e3_session *s, const float *vec_h, const void *feats_h, const void *weights_h,
                                    const int32_t *senders_h, const int32_t *receivers_h, int64_t n_edges, int32_t n_nodes,
                                    const float *grad_out_h, float *out_h, float *grad_feats_h, void *grad_weights_h,
                                    float *grad_vec_h, float *forces_h, int64_t *bytes_h2d, int64_t *bytes_d2h)
@@ -438,6 +438,19 @@ extern "C" int e3_session_run_host(e3_session *s, const float *vec_h, const void
         (n_nodes > 0 && !feats_h) || (n_edges > 0 && (!vec_h || !weights_h || !senders_h || !receivers_h))) {
         set_error("e3_session_run_host: bad arguments or sizes above the session capacity");
         return E3_ERR_INVALID_ARG;
+    }
+    // the index arrays are on the host: range and sortedness are checked here, before anything is launched
+    // (the kernels index row_ptr / col_ptr / feats with them and the chunking below bisects receivers_h)
+    for (int64_t e = 0; e < n_edges; ++e) {
+        const int32_t sv = senders_h[e], rv = receivers_h[e];
+        if (sv < 0 || sv >= n_nodes || rv < 0 || rv >= n_nodes) {
+            set_error("e3_session_run_host: edge %lld has an index out of range [0, %d)", (long long)e, (int)n_nodes);
+            return E3_ERR_INVALID_ARG;
+        }
+        if (e > 0 && rv < receivers_h[e - 1]) {
+            set_error("e3_session_run_host: receivers are not sorted ascending (edge %lld)", (long long)e);
+            return E3_ERR_UNSORTED;
+        }
     }
     const e3_plan *pl = s->plan;
     const size_t E = (size_t)n_edges, N = (size_t)n_nodes, es = esize(pl), P = pl->paths.size(), C = pl->C;
@@ -511,4 +524,20 @@ extern "C" int e3_session_run_host(e3_session *s, const float *vec_h, const void
     if (bytes_h2d) *bytes_h2d = up;
     if (bytes_d2h) *bytes_d2h = down;
     return E3_OK;
+}
+
+extern "C" int e3_session_run_host(e3_session *s, const float *vec_h, const void *feats_h, const void *weights_h,
+                                   const int32_t *senders_h, const int32_t *receivers_h, int64_t n_edges, int32_t n_nodes,
+                                   const float *grad_out_h, float *out_h, float *grad_feats_h, void *grad_weights_h,
+                                   float *grad_vec_h, float *forces_h, int64_t *bytes_h2d, int64_t *bytes_d2h)
+{
+    const int rc = session_run_host_impl(s, vec_h, feats_h, weights_h, senders_h, receivers_h, n_edges, n_nodes, grad_out_h, out_h,
+                                         grad_feats_h, grad_weights_h, grad_vec_h, forces_h, bytes_h2d, bytes_d2h);
+    if (rc != E3_OK && s) {      // no asynchronous copy may still touch the caller's host buffers after a failing return
+        cudaStreamSynchronize(s->stream_in);
+        cudaStreamSynchronize(s->stream);
+        cudaStreamSynchronize(s->stream_out);
+        cudaGetLastError();
+    }
+    return rc;
 }

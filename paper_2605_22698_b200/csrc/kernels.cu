@@ -212,20 +212,44 @@ __global__ void graph_fill_kernel(const int32_t *__restrict__ snd, int64_t E, in
     if (e < E) fill[atomicAdd(&cursor[snd[e]], 1)] = (int32_t)e;
 }
 
-// one warp per sender: rank-sort its (arbitrarily ordered) segment of edge ids ascending
-__global__ void graph_segment_sort_kernel(const int32_t *__restrict__ col_ptr, const int32_t *__restrict__ fill,
+// one warp per sender: sort its (arbitrarily ordered) segment of edge ids ascending.  Short segments (the common case,
+// degree ~50) are rank-sorted, O(deg^2 / 32) per lane; long ones (hub senders) by a bottom-up merge sort that ping-pongs
+// between `fill` and `perm_s`, every element finding its place in the merged run by binary search in the sibling run
+// (edge ids are unique, so the result is the unique ascending order either way).
+__global__ void graph_segment_sort_kernel(const int32_t *__restrict__ col_ptr, int32_t *__restrict__ fill,
                                           int32_t N, int32_t *__restrict__ perm_s)
 {
     int32_t s = (int32_t)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
     if (s >= N) return;
     const int lane = threadIdx.x & 31;
     const int32_t a = col_ptr[s], b = col_ptr[s + 1];
-    for (int32_t i = a + lane; i < b; i += 32) {
-        int32_t v = fill[i];
-        int32_t rank = 0;
-        for (int32_t j = a; j < b; ++j) rank += (fill[j] < v);
-        perm_s[a + rank] = v;
+    const int32_t n = b - a;
+    if (n <= 128) {
+        for (int32_t i = a + lane; i < b; i += 32) {
+            int32_t v = fill[i];
+            int32_t rank = 0;
+            for (int32_t j = a; j < b; ++j) rank += (fill[j] < v);
+            perm_s[a + rank] = v;
+        }
+        return;
     }
+    int32_t *src = fill + a, *dst = perm_s + a;
+    for (int32_t width = 1; width < n; width <<= 1) {
+        for (int32_t i = lane; i < n; i += 32) {
+            const int32_t base = (i / (2 * width)) * (2 * width);
+            const int32_t mid = min(base + width, n), end = min(base + 2 * width, n);
+            const int32_t v = src[i];
+            int32_t lo, hi, pos;
+            if (i < mid) { lo = mid; hi = end; } else { lo = base; hi = mid; }
+            while (lo < hi) { const int32_t m = (lo + hi) >> 1; if (src[m] < v) lo = m + 1; else hi = m; }   // #sibling elements < v
+            if (i < mid) pos = i + (lo - mid); else pos = (i - mid) + base + (lo - base);
+            dst[pos] = v;
+        }
+        __syncwarp();
+        int32_t *t = src; src = dst; dst = t;
+    }
+    if (src != perm_s + a)
+        for (int32_t i = lane; i < n; i += 32) perm_s[a + i] = src[i];
 }
 
 int launch_graph_prepare(const int32_t *snd, const int32_t *rcv, int64_t E, int32_t N, int32_t *row_ptr,

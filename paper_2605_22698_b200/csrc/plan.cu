@@ -142,16 +142,20 @@ int launch_cg_planner(const int *triples, int n, std::vector<std::vector<double>
     int total = off[n];
     int *d_tr = nullptr, *d_off = nullptr;
     double *d_dense = nullptr;
-    E3_CUDA_TRY(cudaMalloc(&d_tr, sizeof(int) * 3 * n));
-    E3_CUDA_TRY(cudaMalloc(&d_off, sizeof(int) * (n + 1)));
-    E3_CUDA_TRY(cudaMalloc(&d_dense, sizeof(double) * total));
-    E3_CUDA_TRY(cudaMemcpy(d_tr, triples, sizeof(int) * 3 * n, cudaMemcpyHostToDevice));
-    E3_CUDA_TRY(cudaMemcpy(d_off, off.data(), sizeof(int) * (n + 1), cudaMemcpyHostToDevice));
-    cg_planner_kernel<<<(total + 127) / 128, 128>>>(d_tr, d_off, n, total, d_dense);
-    E3_CUDA_TRY(cudaGetLastError());
     std::vector<double> flat(total);
-    E3_CUDA_TRY(cudaMemcpy(flat.data(), d_dense, sizeof(double) * total, cudaMemcpyDeviceToHost));
-    cudaFree(d_tr); cudaFree(d_off); cudaFree(d_dense);
+    // legacy default stream + blocking copies: e3_plan_create is documented to synchronise
+    cudaError_t e = cudaMalloc(&d_tr, sizeof(int) * 3 * n);
+    if (e == cudaSuccess) e = cudaMalloc(&d_off, sizeof(int) * (n + 1));
+    if (e == cudaSuccess) e = cudaMalloc(&d_dense, sizeof(double) * total);
+    if (e == cudaSuccess) e = cudaMemcpy(d_tr, triples, sizeof(int) * 3 * n, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(d_off, off.data(), sizeof(int) * (n + 1), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        cg_planner_kernel<<<(total + 127) / 128, 128>>>(d_tr, d_off, n, total, d_dense);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(flat.data(), d_dense, sizeof(double) * total, cudaMemcpyDeviceToHost);
+    cudaFree(d_tr); cudaFree(d_off); cudaFree(d_dense);      // on every path
+    if (e != cudaSuccess) return cuda_fail(e, "cg planner");
     dense_out.resize(n);
     for (int t = 0; t < n; ++t) dense_out[t].assign(flat.begin() + off[t], flat.begin() + off[t + 1]);
     return E3_OK;
@@ -285,17 +289,29 @@ void plan_make_roles(e3_plan &pl)
         total_cost += cost[o];
         total_rows += 2 * pl.irreps_out[o].l + 1;
     }
-    // tuning aid: E3_TUNE="key=value,..." overrides launch-shape heuristics (never changes results)
-    pl.v2 = v2_eligible(pl) ? 1 : 0;
-    { const char *t = getenv("E3_TUNE"); if (t && strstr(t, "v2=0")) pl.v2 = 0; }
-    int rows_target = 20, rows_hard = pl.v2 ? 22 : 28;
+    // tuning aid: E3_TUNE="key=value,..." overrides launch-shape heuristics (never changes results).  The string is
+    // tokenised on ',' and whole keys are matched (so "bwd_v2=0" does not also set "v2"); the last occurrence wins.
     const char *tune = getenv("E3_TUNE");
+    std::map<std::string, int> tune_map;
+    if (tune) {
+        std::string t(tune);
+        size_t a = 0;
+        while (a <= t.size()) {
+            size_t b = t.find(',', a);
+            if (b == std::string::npos) b = t.size();
+            std::string tok = t.substr(a, b - a);
+            size_t eq = tok.find('=');
+            if (eq != std::string::npos && eq > 0) tune_map[tok.substr(0, eq)] = atoi(tok.c_str() + eq + 1);
+            a = b + 1;
+        }
+    }
     auto tune_get = [&](const char *key, int &dst) {
-        if (!tune) return;
-        std::string t(tune), k = std::string(key) + "=";
-        size_t pos = t.find(k);
-        if (pos != std::string::npos && (pos == 0 || t[pos - 1] == ',')) dst = atoi(t.c_str() + pos + k.size());
+        auto it = tune_map.find(key);
+        if (it != tune_map.end()) dst = it->second;
     };
+    pl.v2 = v2_eligible(pl) ? 1 : 0;
+    { int v2 = 1; tune_get("v2", v2); if (!v2) pl.v2 = 0; }
+    int rows_target = 20, rows_hard = pl.v2 ? 22 : 28;
     tune_get("rows", rows_target); tune_get("rows_hard", rows_hard);
     if (rows_hard < rows_target) rows_hard = rows_target + 8;
     int n_roles = std::max(1, (total_rows + rows_target - 1) / rows_target);

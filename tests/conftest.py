@@ -10,15 +10,22 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
+    config.addinivalue_line("markers", "sanitizer: runs a tiny case under compute-sanitizer (one tool per gpurun call; run explicitly)")
 
 
 def pytest_collection_modifyitems(config, items):
+    # `sanitizer` cases run only when asked for by name (-m sanitizer): one compute-sanitizer tool per gpurun call
+    if "sanitizer" not in (config.getoption("-m") or ""):
+        drop = [it for it in items if "sanitizer" in it.keywords]
+        if drop:
+            items[:] = [it for it in items if "sanitizer" not in it.keywords]
+            config.hook.pytest_deselected(items=drop)
     import torch
     if torch.cuda.is_available():
         return
     skip = pytest.mark.skip(reason="no CUDA device")
     for it in items:
-        if "gpu" in it.keywords:
+        if "gpu" in it.keywords or "sanitizer" in it.keywords:
             it.add_marker(skip)
 
 

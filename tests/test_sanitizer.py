@@ -1,0 +1,41 @@
+"""compute-sanitizer gate (SURVEY section 4 T4 / section 5 "race detection"): the generated kernels rely on hand-derived
+invariants (a lane reads back only what it copied; static cp.async.wait_group counts; ring memory reused for the fsplit
+partial sums), which parity tests cannot see.  Marker `sanitizer`, NOT `gpu`: B200_PROFILING.md allows one compute-sanitizer
+tool per gpurun call, so the driver's `-m gpu` run deselects this file and it is run explicitly,
+
+    E3_SAN_TOOL=racecheck python -m pytest tests/test_sanitizer.py -m sanitizer -q
+
+one tool per call (default racecheck).  The summaries of those runs are committed in profiles/r02_sanitizer.md."""
+import os
+import re
+import shutil
+import subprocess
+import sys
+
+import pytest
+
+pytestmark = pytest.mark.sanitizer
+HERE = os.path.dirname(os.path.abspath(__file__))
+TOOL = os.environ.get("E3_SAN_TOOL", "racecheck")
+CASES = [("smoke", ""), ("ring", ""), ("ragged64", "fwd_split=4,bwd_split=3"), ("ragged128", "bwd_depth=1,bwd_r=2"),
+         ("ragged32", "v2=0"), ("bf16_64", ""), ("degenerate", "")]
+
+
+@pytest.mark.parametrize("case,tune", CASES)
+def test_compute_sanitizer_reports_no_error(case, tune):
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    san = shutil.which("compute-sanitizer") or "/usr/local/cuda/bin/compute-sanitizer"
+    cmd = [san, "--tool", TOOL, "--print-limit", "20", "--error-exitcode", "77"]
+    if TOOL == "racecheck":
+        cmd += ["--racecheck-report", "all"]
+    cmd += [sys.executable, os.path.join(HERE, "sanitizer_case.py"), case, tune]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=1500)
+    text = r.stdout + r.stderr
+    tail = "\n".join(text.strip().splitlines()[-25:])
+    print(f"[{TOOL}] {case} {tune!r} rc={r.returncode}\n{tail}")
+    assert r.returncode == 0, tail
+    m = re.search(r"(ERROR SUMMARY|RACECHECK SUMMARY): (\d+) (error|hazard)", text)
+    assert m is not None and int(m.group(2)) == 0, tail
+    assert "sanitizer_case " + case in text
