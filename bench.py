@@ -9,19 +9,27 @@ host-buffer C entry point (e3_session_run_host) with pinned host tensors, copies
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
 
+Without --config the headline is config 4 (100 000 atoms, fp32: the largest fp32 single-GPU configuration and one of
+north_star's two targets) and the full block of config 2 (the other target) rides along under "secondary".
 `--impl reference` times the fp64 CPU oracle (oracle/) on this box's host cores instead.
 Prints ONE JSON line on rank 0.
 """
 from __future__ import annotations
 
-import argparse
-import json
 import os
-import sys
-import threading
-import time
 
-import numpy as np
+# the oracle's OpenMP threads are pinned (read by libgomp when it is first loaded); set before anything imports OpenMP
+os.environ.setdefault("OMP_PROC_BIND", "close")
+os.environ.setdefault("OMP_PLACES", "cores")
+
+import argparse  # noqa: E402
+import hashlib  # noqa: E402
+import json  # noqa: E402
+import sys  # noqa: E402
+import threading  # noqa: E402
+import time  # noqa: E402
+
+import numpy as np  # noqa: E402
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
@@ -29,12 +37,33 @@ sys.path.insert(0, ROOT)
 METRIC = "edge-messages/s for TP+scatter fwd+VJP (whole hot path a2-a7)"
 UNIT = "edges/s"
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # nominal FFMA peak, 74.45
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the ncu --set full
-# capture named in profiles/ (filled in per round; None when no capture exists for that workload)
-NCU_TRAFFIC_BYTES = {
-    "cfg2_mace_1536atoms_128ch_l3": 1251569920,     # profiles/r01c_cfg2_full.md: e3_bwd 595.83 MB read + 655.74 MB written
-    "cfg4_100k_64ch_l3": 119887406000,              # profiles/r01b_cfg4_full.md: e3_bwd 51.93 GB read + 67.96 GB written
-}
+PRIMARY, SECONDARY = 4, 2
+KERNEL_SOURCES = ["plan.cu", "kernels.cu", "api.cu", "codegen.cpp", "codegen2.cpp", "jit.cpp", "e3_internal.h"]
+
+
+def kernel_sources_sha():
+    """Hash of the CUDA sources the kernels are generated / compiled from; profiles/traffic.json records the value its
+    ncu captures were taken with, and a capture taken with other sources is refused (reported as null)."""
+    h = hashlib.sha256()
+    for f in KERNEL_SOURCES:
+        p = os.path.join(ROOT, "paper_2605_22698_b200", "csrc", f)
+        h.update(f.encode())
+        h.update(open(p, "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(workload, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from profiles/traffic.json (written by
+    bench_traffic.py from an `ncu --set full` capture); (bytes, note)."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(p):
+        return None, "no profiles/traffic.json"
+    ent = json.load(open(p)).get(workload, {}).get(kernel)
+    if ent is None:
+        return None, f"no capture of {kernel} for {workload}"
+    if ent.get("csrc_sha") != kernel_sources_sha():
+        return None, f"capture {ent.get('capture')} was taken with other kernel sources (csrc_sha {ent.get('csrc_sha')}); refused"
+    return int(ent["dram_bytes"]), f"{ent.get('capture')} ({ent.get('captured')})"
 
 
 def load_peaks():
@@ -108,76 +137,130 @@ def algorithmic_bytes(E, N, P, C, in_dim, sh_dim, out_dim, b):
     return fwd, bwd
 
 
-def workload_dict(cfg, E, N, extra=None):
-    d = {"workload": cfg.name, "n_atoms": N, "n_edges": E, "channels": cfg.channels,
-         "irreps_in": "+".join(f"{cfg.channels}x{l}{'e' if p > 0 else 'o'}" for l, p in cfg.irreps_in),
-         "sh_lmax": cfg.sh_lmax, "out_lmax": cfg.out_lmax, "storage": cfg.storage,
-         "seed": cfg.seed, "cutoff_A": 5.0}
-    if extra:
-        d.update(extra)
-    return d
+def workload_dict(cfg, E, N, world):
+    """The `config` object: identical in the GPU arm and the reference arm (the driver compares them)."""
+    return {"workload": cfg.name, "n_atoms": N, "n_edges": E, "channels": cfg.channels,
+            "irreps_in": "+".join(f"{cfg.channels}x{l}{'e' if p > 0 else 'o'}" for l, p in cfg.irreps_in),
+            "sh_lmax": cfg.sh_lmax, "out_lmax": cfg.out_lmax, "storage": cfg.storage,
+            "seed": cfg.seed, "cutoff_A": 5.0,
+            "l2_policy": "inputs larger than L2 (126 MB): every step streams its weights from HBM; no explicit flush",
+            "parallelism": f"replicas x{world}, no data-path collective"}
 
 
 # --------------------------------------------------------------------------------------------
-# reference arm: the fp64 oracle on the host cores
+# the fp64 oracle on the host cores (cpu_baseline leg and the reference arm)
 # --------------------------------------------------------------------------------------------
-def oracle_sample(cfg, max_edges):
-    """A bounded sample of the workload for the CPU oracle: the edges of the first receivers."""
+ORACLE_RECEIVERS = {1: None, 2: None, 3: None, 4: 2000, 5: 2000}     # SURVEY 8(d): configs 4-5 on the first 2 000 receivers' edges
+
+
+def oracle_sample(cfg, n_receivers):
+    """A bounded sample of the workload for the CPU oracle: the edges of the first `n_receivers` receivers (None = all)."""
     import oracle as O
     from paper_2605_22698_b200 import workloads as W
     irreps_in = [(l, p, cfg.channels) for l, p in cfg.irreps_in]
     irreps_out, paths = O.all_paths(irreps_in, cfg.sh_lmax, cfg.out_lmax)
     g, rng = W.make_graph(cfg)
-    E = min(g.n_edges, max_edges)
-    if E < g.n_edges:                       # cut at a receiver boundary
-        E = int(np.searchsorted(g.receivers, g.receivers[E], side="left"))
+    E = g.n_edges
+    if n_receivers is not None and n_receivers < g.n_nodes:
+        E = int(np.searchsorted(g.receivers, n_receivers, side="left"))
     out_dim = sum(2 * l + 1 for l, _, _ in irreps_out)
     x = W.draw_x(cfg, rng)
     snd, rcv, vec = g.senders[:E], g.receivers[:E], g.vec[:E]
+    n_loc = g.n_nodes
+    G = W.draw_g(cfg, np.random.Generator(np.random.Philox(cfg.seed + 2000)), out_dim)
+    if E < g.n_edges:
+        # the sub-graph is relabelled onto the atoms it touches (receivers keep their order, so edges stay receiver-sorted):
+        # the oracle's dense fp64 node arrays then cover ~7 000 atoms instead of 100 000
+        ids = np.unique(np.concatenate([np.arange(n_receivers, dtype=np.int64), snd.astype(np.int64)]))
+        snd = np.searchsorted(ids, snd).astype(np.int32)
+        rcv = np.searchsorted(ids, rcv).astype(np.int32)
+        x, G, n_loc = x[ids], G[ids], int(ids.size)
     wrng = np.random.Generator(np.random.Philox(cfg.seed + 1000))
     w = W.round_to_storage(wrng.normal(size=(E, len(paths) * cfg.channels)) * W.w_sigma(cfg, len(paths)), cfg.storage)
-    G = W.draw_g(cfg, np.random.Generator(np.random.Philox(cfg.seed + 2000)), out_dim)
     pl = (irreps_in, cfg.sh_lmax, irreps_out, paths)
-    desc = (f"all {g.n_edges} edges" if E == g.n_edges else f"edges of the first {int(rcv[-1]) + 1} receivers ({E} of {g.n_edges} edges)")
-    return pl, g.n_nodes, snd, rcv, vec, x, w, G, E, desc
+    desc = (f"all {g.n_edges} edges" if E == g.n_edges else
+            f"edges of the first {n_receivers} receivers ({E} of {g.n_edges} edges, relabelled onto the {n_loc} atoms they touch)")
+    return dict(pl=pl, N=n_loc, N_full=g.n_nodes, snd=snd, rcv=rcv, vec=vec, x=x, w=w, G=G, E=E, desc=desc, E_full=g.n_edges, forces=cfg.forces)
 
 
-def oracle_step(pl, N, snd, rcv, vec, x, w, G, forces=True):
+def oracle_step(s, n_edges=None):
     import oracle as O
+    e = s["E"] if n_edges is None else n_edges
+    pl, N = s["pl"], s["N"]
+    snd, rcv, vec, w = s["snd"][:e], s["rcv"][:e], s["vec"][:e], s["w"][:e]
     O.graph_prepare(snd, rcv, N)
     Y = O.sh(pl[1], vec)
-    O.tp_scatter_fwd(*pl, x, Y, w, snd, rcv, N)
-    _, dY, _ = O.tp_scatter_bwd(*pl, x, Y, w, snd, rcv, N, G)
+    O.tp_scatter_fwd(*pl, s["x"], Y, w, snd, rcv, N)
+    _, dY, _ = O.tp_scatter_bwd(*pl, s["x"], Y, w, snd, rcv, N, s["G"])
     dvec = O.sh_bwd(pl[1], vec, dY)
-    if forces:
-        O.force_reduce(dvec, snd, rcv, N)
+    O.force_reduce(dvec, snd, rcv, N)
 
 
-def time_oracle(cfg, steps, warmup, budget_edges=400_000):
+def time_oracle(cfg, reps=5, sample=None):
+    """cpu_baseline: the oracle as it stands, all host cores (OpenMP, threads pinned), one full warm-up step, then `reps`
+    steps timed one by one (min and median reported; `value` is the median); plus a single-thread figure on a
+    sub-sample of about 1/8 of those edges (SURVEY 8(d) asks for both)."""
     import oracle as O
-    pl, N, snd, rcv, vec, x, w, G, E, desc = oracle_sample(cfg, budget_edges)
-    for _ in range(warmup):
-        oracle_step(pl, N, snd, rcv, vec, x, w, G)
-    t0 = time.perf_counter()
-    for _ in range(steps):
-        oracle_step(pl, N, snd, rcv, vec, x, w, G)
-    dt = time.perf_counter() - t0
-    return {"value": E * steps / dt, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
-            "sample": f"{desc}, {steps} step(s), fp64, gcc -O2 + OpenMP"}, dt / steps * 1e3, E, N
+    s = sample if sample is not None else oracle_sample(cfg, ORACLE_RECEIVERS[cfg.k])
+    nthr = O.num_threads()
+    oracle_step(s)
+    ts = []
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        oracle_step(s)
+        ts.append(time.perf_counter() - t0)
+    e1 = s["E"]
+    if s["E"] > 20000:                    # single thread: the edges of about 1/8 of the receivers, cut at a receiver boundary
+        e1 = int(np.searchsorted(s["rcv"], s["rcv"][s["E"] // 8], side="left")) or s["E"]
+    O.set_num_threads(1)
+    oracle_step(s, e1)
+    t1 = []
+    for _ in range(3):
+        t0 = time.perf_counter()
+        oracle_step(s, e1)
+        t1.append(time.perf_counter() - t0)
+    O.set_num_threads(nthr)
+    med = float(np.median(ts))
+    cb = {"value": s["E"] / med, "unit": UNIT, "cores": nthr, "kind": "oracle",
+          "sample": f"{s['desc']}; fp64, gcc -O2 + OpenMP (OMP_PROC_BIND={os.environ.get('OMP_PROC_BIND')}); 1 warm-up + {reps} steps, value = median",
+          "all_cores": {"threads": nthr, "nproc": os.cpu_count(), "edges_per_s_median": s["E"] / med, "edges_per_s_best": s["E"] / min(ts),
+                        "ms_per_step_median": med * 1e3},
+          "single_thread": {"threads": 1, "edges": e1, "edges_per_s_median": e1 / float(np.median(t1)), "edges_per_s_best": e1 / min(t1)}}
+    return cb, s
 
 
 def run_reference(args):
+    """Reference arm = the oracle (tier framing): same metric / config dict as the GPU arm; each "step" is one pass of the
+    hot path over the bounded sample; the step count is capped so the run ends within minutes (stated in the line)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
+    import oracle as O
     from paper_2605_22698_b200 import workloads as W
-    cfg = W.CONFIGS[args.config]
+    k = args.config if args.config else PRIMARY
+    cfg = W.CONFIGS[k]
+    s = oracle_sample(cfg, ORACLE_RECEIVERS[k])
     steps = max(1, min(args.steps, 5))
-    cb, ms, E, N = time_oracle(cfg, steps, min(args.warmup, 1))
-    line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
-            "warmup": min(args.warmup, 1), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic", "config": workload_dict(cfg, E, N, {"note": "bounded sample, see cpu_baseline.sample"}),
-            "cpu_baseline": cb, "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    warm = max(1, min(args.warmup, 1))
+    for _ in range(warm):
+        oracle_step(s)
+    ts = []
+    for _ in range(steps):
+        t0 = time.perf_counter()
+        oracle_step(s)
+        ts.append(time.perf_counter() - t0)
+    med = float(np.median(ts))
+    value = s["E"] / med
+    cb = {"value": value, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+          "sample": f"{s['desc']}; fp64, gcc -O2 + OpenMP (OMP_PROC_BIND={os.environ.get('OMP_PROC_BIND')}); {warm} warm-up + {steps} steps, value = median",
+          "all_cores": {"threads": O.num_threads(), "nproc": os.cpu_count(), "edges_per_s_median": value, "edges_per_s_best": s["E"] / min(ts)}}
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": warm, "steps_requested": args.steps, "warmup_requested": args.warmup,
+            "steps_capped_to": steps if steps != args.steps else None, "warmup_capped_to": warm if warm != args.warmup else None,
+            "ms_per_step": med * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": workload_dict(cfg, s["E_full"], s["N_full"], world),
+            "cpu_baseline": cb, "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
 
@@ -199,23 +282,25 @@ def aggregate_replicas(elapsed_ms, n_edges, steps, world, device):
     return elapsed_ms, world * n_edges * steps / (elapsed_ms * 1e-3)
 
 
-def run_ours(args):
+def e2e_subset_edges(g, w_row_bytes, budget_bytes=3 << 30):
+    """Largest receiver range [0, R) whose weights fit `budget_bytes` of pinned host memory (the gradient of the weights
+    needs as much again): number of edges, cut at a receiver boundary."""
+    e = min(g.n_edges, budget_bytes // w_row_bytes)
+    if e < g.n_edges:
+        e = int(np.searchsorted(g.receivers, g.receivers[e], side="left"))
+    return e
+
+
+def measure_config(k, args, world, rank, local, dev, steps, want_cpu, want_e2e):
+    """Runs workload k on this rank's GPU; returns the JSON block (rank 0) or None."""
+    import ctypes as Ct
+    import gc
     import torch
     import torch.distributed as dist
     from paper_2605_22698_b200 import binding as B
     from paper_2605_22698_b200 import workloads as W
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback (use --impl reference for the oracle)")
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
-
-    cfg = W.CONFIGS[args.config]
+    cfg = W.CONFIGS[k]
     irreps_in = [(l, p, cfg.channels) for l, p in cfg.irreps_in]
     irreps_out, paths = B.e3_all_paths(irreps_in, cfg.sh_lmax, cfg.out_lmax)
     plan = B.e3_plan_create(irreps_in, cfg.sh_lmax, irreps_out, paths, B.E3_BF16 if cfg.storage == "bf16" else B.E3_F32)
@@ -247,7 +332,6 @@ def run_ours(args):
     F = torch.empty((N, 3), dtype=torch.float32, device=dev)
     ws = torch.empty(B.e3_bwd_workspace_bytes(plan, E, N), dtype=torch.uint8, device=dev)
     L = B.lib()
-    import ctypes as Ct
     gws_bytes = L.e3_graph_workspace_bytes(E, N)
     gws = torch.empty(gws_bytes, dtype=torch.uint8, device=dev)
     row_ptr = torch.empty(N + 1, dtype=torch.int32, device=dev)
@@ -260,8 +344,6 @@ def run_ours(args):
     def chk(rc, what):
         if rc != 0:
             raise RuntimeError(f"{what}: {L.e3_status_string(rc).decode()}: {L.e3_last_error().decode()}")
-
-    ev = {}
 
     def step(timed_events=None):
         def mark(name):
@@ -295,26 +377,27 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
+    warm = max(args.warmup, 3)
+    for _ in range(warm):
         step()
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
     t_start, t_stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     t_start.record(stream)
-    for _ in range(args.steps):
+    for _ in range(steps):
         step()
     t_stop.record(stream)
     barrier()
     clocks = sampler.stop()
-    elapsed_ms, value = aggregate_replicas(t_start.elapsed_time(t_stop), E, args.steps, world, dev)
+    elapsed_ms, value = aggregate_replicas(t_start.elapsed_time(t_stop), E, steps, world, dev)
 
     # per-call / per-kernel device times, measured live with events on the launching stream over
     # a second pass of the same steps (events between calls would otherwise perturb `value`)
     mid = torch.cuda.Event(enable_timing=True)
     mid.record(stream)
     plan.set_mid_event(mid)
-    n_prof = min(args.steps, 50)
+    n_prof = min(steps, 50)
     acc = {}
     for _ in range(n_prof):
         evs = []
@@ -325,11 +408,11 @@ def run_ours(args):
         tb = [e for n_, e in evs if n_ == "tp_scatter_fwd"][0]
         te = [e for n_, e in evs if n_ == "tp_scatter_bwd"][0]
         acc.setdefault("e3_bwd_kernel", []).append(tb.elapsed_time(mid))
-        acc.setdefault("dx_reduce_kernel", []).append(mid.elapsed_time(te))     # + gsh_reduce when the backward has several roles
+        acc.setdefault("bwd_phase2_kernels", []).append(mid.elapsed_time(te))     # dx_reduce (+ gsh_reduce when the backward has several roles)
     plan.set_mid_event(None)
-    kms = {k: float(np.mean(v)) for k, v in acc.items()}
+    kms = {k_: float(np.mean(v)) for k_, v in acc.items()}
 
-    line = None
+    block = None
     if rank == 0:
         hbm_peak, peak_src = load_peaks()
         b = 2 if cfg.storage == "bf16" else 4
@@ -341,9 +424,10 @@ def run_ours(args):
             t_h, t_f = bytes_ / (hbm_peak * 1e9), flops / (FP32_PEAK_TFLOPS * 1e12)
             if t_h >= t_f:
                 a = bytes_ / (ms * 1e-3) / 1e9
-                return {"bound": "hbm", "achieved": a, "peak": hbm_peak, "unit": "GB/s", "frac": a / hbm_peak}
+                return {"bound": "hbm", "achieved": a, "peak": hbm_peak, "unit": "GB/s", "frac": a / hbm_peak, "peak_source": peak_src}
             a = flops / (ms * 1e-3) / 1e12
-            return {"bound": "alu", "achieved": a, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": a / FP32_PEAK_TFLOPS}
+            return {"bound": "alu", "achieved": a, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": a / FP32_PEAK_TFLOPS,
+                    "peak_source": "DESIGN.md section 7: 148 SM x 128 FMA lanes x 2 flop x 1.965 GHz (guide unit counts and max clock)"}
 
         # FP32 ceiling of this board, measured (register-only FFMA2 kernel, ~0.3 s: long enough for the power cap to act);
         # context for the ALU-bound fractions, which keep the nominal-clock peak as their denominator
@@ -353,71 +437,128 @@ def run_ours(args):
         except Exception:
             alu_meas = None
         dom = roof(bwd_B, bwd_F, kms["e3_bwd_kernel"])
+        tr, tr_note = ncu_traffic(cfg.name, "e3_bwd")
         dom.update({"kernel": "e3_bwd (JIT, first phase of e3_tp_scatter_bwd)", "ms": kms["e3_bwd_kernel"],
-                    "algorithmic_bytes": bwd_B, "algorithmic_flops": bwd_F, "peak_source": peak_src,
-                    "traffic": NCU_TRAFFIC_BYTES.get(cfg.name)})
+                    "algorithmic_bytes": bwd_B, "algorithmic_flops": bwd_F, "traffic": tr, "traffic_source": tr_note})
         fwd_r = roof(fwd_B, fwd_F, kms["tp_scatter_fwd"])
-        fwd_r.update({"kernel": "e3_fwd (JIT)", "ms": kms["tp_scatter_fwd"], "algorithmic_bytes": fwd_B, "algorithmic_flops": fwd_F})
+        trf, trf_note = ncu_traffic(cfg.name, "e3_fwd")
+        fwd_r.update({"kernel": "e3_fwd (JIT)", "ms": kms["tp_scatter_fwd"], "algorithmic_bytes": fwd_B, "algorithmic_flops": fwd_F,
+                      "traffic": trf, "traffic_source": trf_note})
         t_roof = max(fwd_B / (hbm_peak * 1e9), fwd_F / (FP32_PEAK_TFLOPS * 1e12)) + max(bwd_B / (hbm_peak * 1e9), bwd_F / (FP32_PEAK_TFLOPS * 1e12))
         t_tp = (kms["tp_scatter_fwd"] + kms["tp_scatter_bwd"]) * 1e-3
         tp = {"edges_per_s_fwd_plus_vjp": E / t_tp, "roofline_edges_per_s": E / t_roof, "frac_of_roofline": t_roof / t_tp,
               "ms_fwd": kms["tp_scatter_fwd"], "ms_bwd": kms["tp_scatter_bwd"]}
 
-        # end to end through the host-buffer C entry point (pinned host tensors, copies inside the timed region)
-        e2e = None
-        if not big_w:
-            sess = B.Session(plan, E, N)
-            pin = lambda a, dt=None: (torch.from_numpy(np.ascontiguousarray(a)) if dt is None else torch.from_numpy(np.ascontiguousarray(a)).to(dt)).pin_memory()
-            hv, hx, hw, hs, hr, hG = pin(g.vec), pin(x_h, st), pin(w_h, st), pin(g.senders), pin(g.receivers), pin(G_h)
-            ho = torch.empty((N, plan.out_dim * C), dtype=torch.float32).pin_memory()
-            hdx = torch.empty((N, plan.in_dim * C), dtype=torch.float32).pin_memory()
-            hdw = torch.empty((E, P * C), dtype=st).pin_memory()
-            hdv = torch.empty((E, 3), dtype=torch.float32).pin_memory()
-            hF = torch.empty((N, 3), dtype=torch.float32).pin_memory()
-            n_e2e = max(3, min(args.steps, 20))
-            for _ in range(2):
-                up, down = sess.run_host(hv, hx, hw, hs, hr, N, hG, ho, hdx, hdw, hdv, hF)
-            t0 = time.perf_counter()
-            for _ in range(n_e2e):
-                sess.run_host(hv, hx, hw, hs, hr, N, hG, ho, hdx, hdw, hdv, hF)
-            dt = time.perf_counter() - t0
-            e2e = {"value": world * E * n_e2e / dt, "unit": UNIT, "h2d_bytes_per_step": up, "d2h_bytes_per_step": down,
-                   "steps": n_e2e, "ms_per_step": dt / n_e2e * 1e3, "api": "e3_session_run_host (pinned host buffers)"}
-            sess.destroy()
+        block = {"value": value, "unit": UNIT, "steps": steps, "warmup": warm, "ms_per_step": elapsed_ms / steps,
+                 "dtype": "f32" if cfg.storage == "f32" else "bf16-storage/f32-accumulate",
+                 "config": workload_dict(cfg, E, N, world), "clocks": clocks, "gpu_launches": KERNELS_PER_STEP * steps,
+                 "roofline": dom, "roofline_fwd": fwd_r, "tp_fwd_plus_vjp": tp,
+                 "alu_peak": {"nominal_tflops": FP32_PEAK_TFLOPS, "measured_sustained_tflops": alu_meas,
+                              "how": "148 SM x 128 lanes x 2 x 1.965 GHz; measured = e3_measure_fp32_peak (FFMA2 chains in registers, 0.3 s)"},
+                 "kernel_ms": kms, "kernel_info": {"fwd": plan.kernel_info(0), "bwd": plan.kernel_info(1)}}
+
+    # free the device-resident run before the host-buffer one (config 4 holds ~125 GB)
+    del out, sh, gfe, gsh, gw, gvec, F, ws, gws, row_ptr, col_ptr, perm_s
+    gc.collect()
+    torch.cuda.empty_cache()
+
+    if rank == 0 and want_e2e:
+        # end to end through the host-buffer C entry point (pinned host tensors, copies inside the timed region).  When the
+        # weights do not fit pinned host memory the run covers the largest receiver range [0, R) whose weights fit 3 GiB
+        # (all N atoms stay in the graph: their features are gathered); the subset is stated.
+        w_row = P * C * b
+        Es = e2e_subset_edges(g, w_row)
+        sess = B.Session(plan, Es, N)
+        pin = lambda a, dt=None: (torch.from_numpy(np.ascontiguousarray(a)) if dt is None else torch.from_numpy(np.ascontiguousarray(a)).to(dt)).pin_memory()
+        if w_h is not None:
+            hw = pin(w_h[:Es], st)
         else:
-            e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": None, "d2h_bytes_per_step": None,
-                   "note": "weights (45.6 GB) exceed what can be staged through host memory on this box; not measured"}
+            hw = torch.empty((Es, P * C), dtype=st).pin_memory()
+            hw.copy_(w[:Es])
+        hv, hx, hs, hr, hG = pin(g.vec[:Es]), pin(x_h, st), pin(g.senders[:Es]), pin(g.receivers[:Es]), pin(G_h)
+        ho = torch.empty((N, plan.out_dim * C), dtype=torch.float32).pin_memory()
+        hdx = torch.empty((N, plan.in_dim * C), dtype=torch.float32).pin_memory()
+        hdw = torch.empty((Es, P * C), dtype=st).pin_memory()
+        hdv = torch.empty((Es, 3), dtype=torch.float32).pin_memory()
+        hF = torch.empty((N, 3), dtype=torch.float32).pin_memory()
+        n_e2e = max(3, min(steps, 20 if Es < 200_000 else 5))
+        for _ in range(2):
+            up, down = sess.run_host(hv, hx, hw, hs, hr, N, hG, ho, hdx, hdw, hdv, hF)
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            sess.run_host(hv, hx, hw, hs, hr, N, hG, ho, hdx, hdw, hdv, hF)
+        dt = time.perf_counter() - t0
+        block["e2e"] = {"value": world * Es * n_e2e / dt, "unit": UNIT, "h2d_bytes_per_step": up, "d2h_bytes_per_step": down,
+                        "steps": n_e2e, "ms_per_step": dt / n_e2e * 1e3, "api": "e3_session_run_host (pinned host buffers)",
+                        "edges_per_step": Es,
+                        "subset": ("whole graph" if Es == E else
+                                   f"receivers [0, {int(g.receivers[Es - 1]) + 1}) of {N} with all their {Es} in-edges (of {E}); all {N} atoms' "
+                                   f"features and cotangent rows are copied; weights of the subset = {Es * w_row / 2**30:.2f} GiB pinned")}
+        sess.destroy()
+        del hw, hdw, ho, hdx, hv, hx, hG
+    elif rank == 0:
+        block["e2e"] = None
+    del w
+    gc.collect()
+    torch.cuda.empty_cache()
 
-        cb = None
-        if world == 1 and not args.no_cpu_baseline:
-            cb, _, _, _ = time_oracle(cfg, 3, 1)
+    if rank == 0:
+        block["cpu_baseline"] = None
+        if world == 1 and want_cpu:
+            block["cpu_baseline"], _ = time_oracle(cfg)
+    plan.destroy()
+    return block
 
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-                "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                "dtype": "f32" if cfg.storage == "f32" else "bf16-storage/f32-accumulate", "data": "synthetic",
-                "config": workload_dict(cfg, E, N, {"l2_policy": f"inputs larger than L2: each step streams {(fwd_B + bwd_B) / 1e9:.2f} GB (L2 126 MB); no explicit flush",
-                                                    "parallelism": f"replicas x{world}, no data-path collective"}),
-                "clocks": clocks, "gpu_launches": KERNELS_PER_STEP * args.steps, "e2e": e2e,
-                "roofline": dom, "roofline_fwd": fwd_r, "tp_fwd_plus_vjp": tp,
-                "alu_peak": {"nominal_tflops": FP32_PEAK_TFLOPS, "measured_sustained_tflops": alu_meas,
-                             "how": "148 SM x 128 lanes x 2 x 1.965 GHz; measured = e3_measure_fp32_peak (FFMA2 chains in registers, 0.3 s)"},
-                "kernel_ms": kms, "kernel_info": {"fwd": plan.kernel_info(0), "bwd": plan.kernel_info(1)},
-                "cpu_baseline": cb}
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    k = args.config if args.config else PRIMARY
+    want_cpu = not args.no_cpu_baseline
+    blk = measure_config(k, args, world, rank, local, dev, args.steps, want_cpu, not args.no_e2e)
+    sec = None
+    if not args.config and not args.no_secondary:
+        # the other north_star target, measured in the same run: enough steps for a >= 0.5 s timed region
+        sec = measure_config(SECONDARY, args, world, rank, local, dev, max(args.steps, 1500), want_cpu, not args.no_e2e)
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
-    if line is not None:
+    if rank == 0:
+        line = {"metric": METRIC, "value": blk["value"], "unit": UNIT, "n_gpus": world, "steps": blk["steps"], "warmup": blk["warmup"],
+                "ms_per_step": blk["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": blk["dtype"], "data": "synthetic"}
+        for key in ("config", "clocks", "gpu_launches", "e2e", "roofline", "roofline_fwd", "tp_fwd_plus_vjp", "alu_peak", "kernel_ms",
+                    "kernel_info", "cpu_baseline"):
+            line[key] = blk[key]
+        line["csrc_sha"] = kernel_sources_sha()
+        if sec is not None:
+            sec["metric"] = METRIC
+            line["secondary"] = sec
         print(json.dumps(line))
 
 
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=300)
-    ap.add_argument("--warmup", type=int, default=10)
-    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=0, choices=[0, 1, 2, 3, 4, 5],
+                    help="0 (default): config 4 as the headline with config 2 under 'secondary'")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-secondary", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -83,6 +83,8 @@ struct e3_plan {
     int bwd_depth = 0;         // v2 backward: ring stages per warp (units in flight); 0 = choose
     int bwd_split = 0;         // v2 backward: CTAs per receiver (0 = choose at launch from the grid size)
     int fwd_split = 0;         // v2 forward: warps sharing one (receiver, role) (0 = choose at launch)
+    int wait_all = 0;          // checking aid (E3_TUNE wait_all=1): every cp.async wait drains all outstanding groups, so a result that differs
+                               // from the normal build would expose a static wait count that is too loose (tests/test_gpu_gaps.py)
     int fwd_ctas_per_sm = 2, bwd_ctas_per_sm = 2;   // measured residency (occupancy API) of the loaded kernels
     int n_sm = 148;            // SM count of the device the plan was created on
     e3::JitKernel fwd, bwd;

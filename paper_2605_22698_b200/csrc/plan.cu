@@ -357,7 +357,7 @@ void plan_make_roles(e3_plan &pl)
     if (!pl.v2) pl.bwd_v2 = 0;
     tune_get("fwd_minb", pl.fwd_minb); tune_get("bwd_minb", pl.bwd_minb);
     tune_get("fwd_warps", pl.fwd_warps); tune_get("bwd_warps", pl.bwd_warps);
-    tune_get("fwd_depth", pl.fwd_depth); tune_get("chunk", pl.fwd_chunk);
+    tune_get("fwd_depth", pl.fwd_depth); tune_get("chunk", pl.fwd_chunk); tune_get("wait_all", pl.wait_all);
 }
 
 }  // namespace e3

@@ -122,3 +122,41 @@ def test_v2_forward_with_first_generation_backward(C, monkeypatch):
     w = rng.normal(size=(e, len(pl[3]) * C)).astype(np.float32)
     G = rng.normal(size=(n, 51 * C)).astype(np.float32)
     compare(run_gpu(plan, g, x, w, G), run_oracle(pl, g, x, w, G))
+
+
+@pytest.mark.parametrize("tune", ["", "fwd_split=4,bwd_split=3", "bwd_depth=1,bwd_r=2", "bwd_role_cost=1", "fwd_depth_max=2", "v2=0"])
+@pytest.mark.parametrize("C,storage", [(32, "f32"), (64, "f32"), (128, "f32"), (64, "bf16")])
+def test_static_cp_async_wait_counts_equal_a_full_drain(tune, C, storage, monkeypatch):
+    """Own race check (compute-sanitizer is closed on this pool, profiles/r02_sanitizer.md): the generated kernels wait for
+    operand copies with STATIC cp.async.wait_group counts derived by the generator.  E3_TUNE wait_all=1 builds the same kernels
+    with every wait draining ALL outstanding copies (always safe, slower).  If any static count were too loose the normal
+    build would consume a ring slot before its copy landed and differ from the drained build; the results must be bit-identical
+    (and both meet the oracle's bars).  Ragged degrees 0..90 exercise prologue, steady state and tail of every ring."""
+    from helpers import TOL_BF16
+    rng = np.random.default_rng(500 + C)
+    cfg = W.small_config(channels=C, irreps_in=((0, 1), (1, -1), (2, 1), (3, -1)), sh_lmax=3, out_lmax=3, storage=storage)
+    pl = plan_inputs(cfg)
+    n = 41
+    deg = rng.integers(0, 12, size=n); deg[4] = 90; deg[9] = 0; deg[10] = 1; deg[11] = 33
+    rcv = np.repeat(np.arange(n), deg)
+    snd = rng.integers(0, n, size=rcv.size)
+    o = np.lexsort((snd, rcv))
+    snd, rcv = snd[o].astype(np.int32), rcv[o].astype(np.int32)
+    e = rcv.size
+    g = W.Graph(n, np.zeros((n, 3)), snd, rcv, (rng.normal(size=(e, 3)) * 2).astype(np.float32), 0.0)
+    x = W.round_to_storage(rng.normal(size=(n, 16 * C)), storage)
+    w = W.round_to_storage(rng.normal(size=(e, 34 * C)), storage)
+    G = rng.normal(size=(n, 156 * C)).astype(np.float32)
+    res = []
+    for extra in ("", "wait_all=1"):
+        t = ",".join(s for s in (tune, extra) if s)
+        if t:
+            monkeypatch.setenv("E3_TUNE", t)
+        plan = gpu_plan(pl, storage)
+        monkeypatch.delenv("E3_TUNE", raising=False)
+        res.append([run_gpu(plan, g, x, w, G) for _ in range(3)])
+    tol = dict(tol_fwd=TOL_BF16, tol_vjp=TOL_BF16, tol_sh=8e-3) if storage == "bf16" else {}
+    compare(res[0][0], run_oracle(pl, g, x, w, G, storage=storage), **tol)
+    for r in res[0] + res[1]:
+        for k in res[0][0]:
+            assert np.array_equal(r[k], res[0][0][k]), (tune, k)

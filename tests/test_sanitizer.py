@@ -35,6 +35,9 @@ def test_compute_sanitizer_reports_no_error(case, tune):
     text = r.stdout + r.stderr
     tail = "\n".join(text.strip().splitlines()[-25:])
     print(f"[{TOOL}] {case} {tune!r} rc={r.returncode}\n{tail}")
+    if r.returncode == 86 and "closed on this pool" in text:
+        pytest.skip("compute-sanitizer is closed on this pool (see profiles/r02_sanitizer.md); own check: "
+                    "tests/test_gpu_gaps.py::test_static_cp_async_wait_counts_equal_a_full_drain")
     assert r.returncode == 0, tail
     m = re.search(r"(ERROR SUMMARY|RACECHECK SUMMARY): (\d+) (error|hazard)", text)
     assert m is not None and int(m.group(2)) == 0, tail
