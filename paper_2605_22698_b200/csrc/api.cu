@@ -1,4 +1,5 @@
 // C ABI entry points (include/e3b200.h): argument checking, launches, the host-buffer session.
+#include <algorithm>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -28,6 +29,19 @@ extern "C" const char *e3_status_string(int status)
 
 extern "C" const char *e3_last_error(void) { return get_error(); }
 
+// dynamic shared memory of the third-generation forward when `f` sub-teams share a receiver
+static int v3_smem(const e3_plan *pl, int f)
+{
+    const int ring = f * pl->fwd_v3_depth * pl->fwd_v3_stage, part = (f - 1) * pl->fwd_v3_part;
+    return pl->fwd_v3_bar + (ring > part ? ring : part);
+}
+static int v3_fsplit_max(const e3_plan *pl)
+{
+    int f = 4;
+    while (f > 1 && (v3_smem(pl, f) > 227 * 1024 || pl->fwd_tw * 32 * f > 1024)) f >>= 1;
+    return f;
+}
+
 // ---------------------------------------------------------------------------------------------
 // plan
 // ---------------------------------------------------------------------------------------------
@@ -36,9 +50,9 @@ static int plan_generate(e3_plan &pl, const char *src_path)
     plan_make_roles(pl);
     pl.fwd.name = "e3_fwd";
     pl.bwd.name = "e3_bwd";
-    pl.fwd.source = pl.v2 ? gen_forward_v2(pl) : gen_forward_source(pl);
+    pl.fwd.source = pl.fwd_v3 ? gen_forward_v3(pl) : (pl.v2 ? gen_forward_v2(pl) : gen_forward_source(pl));
     pl.bwd.source = pl.bwd_v2 ? gen_backward_v2(pl) : gen_backward_source(pl);
-    pl.fwd.threads = pl.fwd_warps * 32;
+    pl.fwd.threads = pl.fwd_v3 ? pl.fwd_tw * 32 : pl.fwd_warps * 32;
     pl.bwd.threads = pl.bwd_warps * 32;
     std::string f1, f2;
     if (src_path) { f1 = std::string(src_path) + ".fwd.cu"; f2 = std::string(src_path) + ".bwd.cu"; }
@@ -64,9 +78,16 @@ extern "C" int e3_plan_create(e3_plan **plan, const e3_irrep *irreps_in, int n_i
     if (rc == E3_OK) rc = plan_generate(*pl, nullptr);
     if (rc == E3_OK) rc = jit_load(pl->fwd);
     if (rc == E3_OK) rc = jit_load(pl->bwd);
-    if (rc == E3_OK && pl->fwd.smem_dyn > 48 * 1024 &&
-        cudaFuncSetAttribute((const void *)pl->fwd.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, pl->fwd.smem_dyn) != cudaSuccess)
+    const int fwd_smem_max = (rc == E3_OK && pl->fwd_v3) ? v3_smem(pl, v3_fsplit_max(pl)) : pl->fwd.smem_dyn;
+    if (rc == E3_OK && fwd_smem_max > 48 * 1024 &&
+        cudaFuncSetAttribute((const void *)pl->fwd.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, fwd_smem_max) != cudaSuccess)
         rc = cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(fwd smem)");
+    if (rc == E3_OK && pl->fwd_v3) {       // zeros: the operands of the missing edges of a receiver's last step
+        pl->zeros_bytes = (size_t)std::max(pl->in_dim, (int)pl->paths.size()) * pl->C * 4 + 256;
+        cudaError_t e = cudaMalloc(&pl->zeros, pl->zeros_bytes);
+        if (e == cudaSuccess) e = cudaMemset(pl->zeros, 0, pl->zeros_bytes);
+        if (e != cudaSuccess) rc = cuda_fail(e, "plan zeros buffer");
+    }
     if (rc == E3_OK && pl->bwd.smem_dyn > 48 * 1024 &&
         cudaFuncSetAttribute((const void *)pl->bwd.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, pl->bwd.smem_dyn) != cudaSuccess)
         rc = cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(bwd smem)");
@@ -78,7 +99,7 @@ extern "C" int e3_plan_create(e3_plan **plan, const e3_irrep *irreps_in, int n_i
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, (const void *)pl->bwd.fn, pl->bwd.threads, pl->bwd.smem_dyn) == cudaSuccess && b > 0) pl->bwd_ctas_per_sm = b;
         cudaGetLastError();
     }
-    if (rc != E3_OK) { jit_unload(pl->fwd); jit_unload(pl->bwd); delete pl; return rc; }
+    if (rc != E3_OK) { jit_unload(pl->fwd); jit_unload(pl->bwd); if (pl->zeros) cudaFree(pl->zeros); delete pl; return rc; }
     *plan = pl;
     return E3_OK;
 }
@@ -88,6 +109,7 @@ extern "C" int e3_plan_destroy(e3_plan *plan)
     if (!plan) return E3_OK;
     jit_unload(plan->fwd);
     jit_unload(plan->bwd);
+    if (plan->zeros) cudaFree(plan->zeros);
     delete plan;
     return E3_OK;
 }
@@ -212,6 +234,29 @@ static int launch_fwd(const e3_plan *plan, const void *feats, const void *sh, co
     // several times over; the result depends on fsplit only through the (fixed) summation grouping
     int fsplit = 1;
     const long long nchb = plan->v2 ? plan->nchb2 : plan->nchb;
+    if (plan->fwd_v3) {
+        // one CTA per (receiver, team, channel block); small graphs: `fsplit` sub-teams share a receiver (each takes a
+        // contiguous run of its edge steps, partial sums added in sub-team order), so that the grid still covers the
+        // machine several times over
+        const long long nteams = (long long)plan->teams.size();
+        fsplit = plan->fwd_split;
+        if (fsplit <= 0) {
+            const double waves = (double)heur_nodes * nteams * nchb / ((double)plan->n_sm * plan->fwd_ctas_per_sm);
+            fsplit = waves >= 6.0 ? 1 : (waves >= 3.0 ? 2 : 4);
+        }
+        if (fsplit != 1 && fsplit != 2 && fsplit != 4) fsplit = 1;
+        const int fmax = v3_fsplit_max(plan);
+        if (fsplit > fmax) fsplit = fmax;
+        const long long chunk_sz = plan->fwd_v3_chunk < n_nodes ? plan->fwd_v3_chunk : n_nodes;
+        const long long chunks = ((long long)n_nodes + chunk_sz - 1) / chunk_sz;
+        const long long grid3 = chunks * chunk_sz * nteams * nchb;
+        if (grid3 > 0x7fffffffLL) { set_error("grid too large"); return E3_ERR_UNSUPPORTED; }
+        const void *zeros = plan->zeros;
+        int chunk_i = (int)chunk_sz;
+        void *args3[] = { (void *)&feats, (void *)&sh, (void *)&weights, (void *)&senders, (void *)&row_ptr, (void *)&out, (void *)&n_nodes, (void *)&fsplit, (void *)&zeros, (void *)&chunk_i };
+        E3_CUDA_TRY(cudaLaunchKernel((const void *)plan->fwd.fn, dim3((unsigned)grid3), dim3(plan->fwd_tw * 32 * fsplit), args3, v3_smem(plan, fsplit), st));
+        return E3_OK;
+    }
     if (plan->v2) {
         fsplit = plan->fwd_split;
         if (fsplit <= 0) {

@@ -83,6 +83,19 @@ struct e3_plan {
     int bwd_depth = 0;         // v2 backward: ring stages per warp (units in flight); 0 = choose
     int bwd_split = 0;         // v2 backward: CTAs per receiver (0 = choose at launch from the grid size)
     int fwd_split = 0;         // v2 forward: warps sharing one (receiver, role) (0 = choose at launch)
+    // third-generation forward (codegen2.cpp gen_forward_v3): a CTA = the roles ("team") of ONE receiver; operands arrive by
+    // TMA bulk copies (cp.async.bulk + mbarrier), the team's sender rows once per edge instead of once per role
+    int fwd_v3 = 0;
+    int fwd_tw = 3;            // warps (roles) per team at most
+    int fwd_v3_depth = 0;      // ring stages per team (0 = choose)
+    int fwd_v3_bulk = 0;       // 1: operands by cp.async.bulk (one elected lane per warp; measured 4.5x slower on config 4: the copies are
+                               // 256 B - 1.8 KB each); 0: per-lane 16-byte cp.async completing on the stage's mbarrier
+    int fwd_v3_lag = 1;        // a stage is refilled `lag` steps after it was consumed (slack between the team's warps)
+    int fwd_v3_stage = 0, fwd_v3_part = 0, fwd_v3_bar = 1024;   // bytes: one ring stage, one sub-team's partial sums, the barrier block
+    int fwd_v3_chunk = 1 << 30;   // receivers per (chunk, team): CTA order is chunk-major, then team (default: team-major, one team's code per SM)
+    std::vector<std::vector<int>> teams;     // role indices per team
+    void *zeros = nullptr;     // device buffer of zeros (source of the operands of a step's missing edges)
+    size_t zeros_bytes = 0;
     int wait_all = 0;          // checking aid (E3_TUNE wait_all=1): every cp.async wait drains all outstanding groups, so a result that differs
                                // from the normal build would expose a static wait count that is too loose (tests/test_gpu_gaps.py)
     int fwd_ctas_per_sm = 2, bwd_ctas_per_sm = 2;   // measured residency (occupancy API) of the loaded kernels
@@ -107,6 +120,8 @@ std::string gen_backward_source(e3_plan &pl);   // also sets pl.bwd.smem_dyn
 bool v2_eligible(const e3_plan &pl);
 std::string gen_forward_v2(e3_plan &pl);
 std::string gen_backward_v2(e3_plan &pl);  // also sets pl.bwd.smem_dyn, pl.bwd_r
+bool v3_eligible(const e3_plan &pl);
+std::string gen_forward_v3(e3_plan &pl);   // sets pl.fwd.smem_dyn (for fsplit = 1), pl.fwd_v3_depth
 
 // jit.cpp
 int jit_compile(JitKernel &k, const std::string &file_hint);   // NVRTC -> cubin (+regs/spill from the ptxas log)

@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <functional>
 #include <map>
 #include <string>
 
@@ -358,6 +359,92 @@ void plan_make_roles(e3_plan &pl)
     tune_get("fwd_minb", pl.fwd_minb); tune_get("bwd_minb", pl.bwd_minb);
     tune_get("fwd_warps", pl.fwd_warps); tune_get("bwd_warps", pl.bwd_warps);
     tune_get("fwd_depth", pl.fwd_depth); tune_get("chunk", pl.fwd_chunk); tune_get("wait_all", pl.wait_all);
+    // third-generation forward: roles aligned with the input irreps, grouped into teams that share one CTA and one copy of
+    // the sender rows per edge
+    tune_get("fwd_v3_bulk", pl.fwd_v3_bulk);
+    pl.fwd_v3 = 0;             // opt-in (E3_TUNE fwd_v3=1): measured no faster than the second generation (experiment viii)
+    tune_get("fwd_v3", pl.fwd_v3);
+    if (!pl.v2 || !v3_eligible(pl)) pl.fwd_v3 = 0;
+    tune_get("team", pl.fwd_tw); tune_get("fwd_v3_depth", pl.fwd_v3_depth); tune_get("fwd_v3_lag", pl.fwd_v3_lag); tune_get("fwd_v3_chunk", pl.fwd_v3_chunk); tune_get("fwd_v3_bulk", pl.fwd_v3_bulk);
+    pl.fwd_tw = std::max(1, std::min(4, pl.fwd_tw));
+    pl.fwd_v3_lag = std::max(1, std::min(2, pl.fwd_v3_lag));
+    if (pl.fwd_v3) {
+        pl.roles.clear();
+        pl.teams.clear();
+        std::vector<std::vector<int>> groups;        // runs of output irreps fed by the same input irrep
+        int last_dom = -2;
+        for (int o : order) {
+            const int dom = feeding[o].empty() ? -1 : pl.paths[first[o]].i_in;
+            if (groups.empty() || dom != last_dom) groups.push_back({});
+            groups.back().push_back(o);
+            last_dom = dom;
+        }
+        // cost of an output irrep in packed 4-channel operations of the factored form (nzM FMAs + the weight multiply) plus its
+        // scalar A entries (one FMUL / FFMA per non-zero, a quarter of a packed operation's pipe time)
+        for (int o : order) {
+            cost[o] = 0.0;
+            for (int p : feeding[o]) {
+                const PathInfo &pi = pl.paths[p];
+                cost[o] += pi.nzM + std::min(2 * pi.l1 + 1, 2 * pi.l3 + 1) + 0.25 * (double)pi.nz.size();
+            }
+        }
+        std::vector<std::vector<int>> group_roles;
+        for (auto &grp : groups) {
+            int rows_g = 0;
+            double cost_g = 0;
+            for (int o : grp) { rows_g += 2 * pl.irreps_out[o].l + 1; cost_g += cost[o]; }
+            const int n_r = std::max(1, (rows_g + rows_hard - 1) / rows_hard);
+            group_roles.push_back({});
+            // contiguous split of the group's output irreps into n_r roles minimising the largest role cost, rows <= rows_hard
+            // per role (more roles if that is infeasible): exact search, the groups are tiny
+            const int n = (int)grp.size();
+            std::vector<int> best_cut;
+            for (int k = n_r; k <= n && best_cut.empty(); ++k) {
+                double best = 1e300;
+                std::vector<int> cut(k + 1, 0);
+                std::function<void(int, int, double)> rec = [&](int part, int start, double worst) {
+                    if (part == k - 1) {
+                        int rows = 0; double c = 0;
+                        for (int i = start; i < n; ++i) { rows += 2 * pl.irreps_out[grp[i]].l + 1; c += cost[grp[i]]; }
+                        if (start >= n || (rows > rows_hard && n - start > 1)) return;
+                        const double wv = std::max(worst, c);
+                        if (wv < best) { best = wv; cut[k] = n; best_cut = cut; }
+                        return;
+                    }
+                    int rows = 0; double c = 0;
+                    for (int end = start + 1; end <= n - (k - 1 - part); ++end) {
+                        rows += 2 * pl.irreps_out[grp[end - 1]].l + 1; c += cost[grp[end - 1]];
+                        if (rows > rows_hard && end - start > 1) break;
+                        cut[part + 1] = end;
+                        rec(part + 1, end, std::max(worst, c));
+                    }
+                };
+                rec(0, 0, 0.0);
+            }
+            if (best_cut.empty()) { best_cut.clear(); for (int i = 0; i <= n; ++i) best_cut.push_back(i); }
+            for (size_t q = 0; q + 1 < best_cut.size(); ++q) {
+                Role cur2; cur2.rows = 0; cur2.cost = 0.0;
+                for (int i = best_cut[q]; i < best_cut[q + 1]; ++i) {
+                    const int o2 = grp[i];
+                    cur2.out_irreps.push_back(o2);
+                    for (int p : feeding[o2]) cur2.paths.push_back(p);
+                    cur2.rows += 2 * pl.irreps_out[o2].l + 1; cur2.cost += cost[o2];
+                }
+                group_roles.back().push_back((int)pl.roles.size());
+                pl.roles.push_back(cur2);
+            }
+        }
+        for (Role &ro : pl.roles) std::sort(ro.paths.begin(), ro.paths.end());
+        std::vector<int> team;
+        for (auto &gr : group_roles) {
+            if (!team.empty() && (int)(team.size() + gr.size()) > pl.fwd_tw) { pl.teams.push_back(team); team.clear(); }
+            for (int ri : gr) {
+                if ((int)team.size() == pl.fwd_tw) { pl.teams.push_back(team); team.clear(); }
+                team.push_back(ri);
+            }
+        }
+        if (!team.empty()) pl.teams.push_back(team);
+    }
 }
 
 }  // namespace e3

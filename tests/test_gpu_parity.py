@@ -211,6 +211,9 @@ def test_vjp_with_arbitrary_sh_input_and_no_grad_weights():
     "bwd_depth=1", "bwd_depth=1,bwd_r=2", "bwd_depth=1,bwd_r=2,bwd_role_cost=1000000",        # ring stages, half-unit weights ring
     "fwd_depth_max=2", "rows=12", "rows=20,rows_hard=30,fwd_minb=2", "chunk=3,bwd_chunk=5",   # forward ring depth, role sizes, CTA order
     "bwd_v2=0", "v2=0",                                                                       # first-generation kernels
+    # third-generation forward (opt-in; team CTAs, mbarrier ring): team shapes, ring depth / lag, CTA order, TMA bulk operand copies
+    "fwd_v3=1", "fwd_v3=1,fwd_v3_lag=2", "fwd_v3=1,team=2", "fwd_v3=1,team=4,fwd_v3_depth=2", "fwd_v3=1,team=1,fwd_v3_chunk=5",
+    "fwd_v3=1,fwd_v3_depth=8,fwd_split=2", "fwd_v3=1,fwd_v3_depth=3,fwd_v3_lag=2,fwd_split=4", "fwd_v3=1,fwd_v3_bulk=1", "fwd_v3=1,fwd_v3_bulk=1,fwd_split=2,team=2",
 ])
 @pytest.mark.parametrize("C", [32, 64, 128])
 def test_launch_shape_variants(tune, C, monkeypatch):
