@@ -18,13 +18,14 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "e3_oracle.c")
+_SRC_NEXT = os.path.join(_HERE, "e3_oracle_next.c")      # SURVEY 8(f) NEXT rows (radial network, second order, ...)
 _LIB = os.path.join(_HERE, "libe3_oracle.so")
 
 
 def build(force: bool = False) -> str:
     """Compile the C oracle with gcc (-O2, no fast-math).  Building the checker is not using it."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", _SRC, "-o", _LIB, "-lm"]
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_NEXT)):
+        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", _SRC, _SRC_NEXT, "-o", _LIB, "-lm"]
         subprocess.run(cmd, check=True)
     return _LIB
 
@@ -198,3 +199,62 @@ def all_paths(irreps_in, sh_lmax, out_lmax, natural_parity_only=False):
                 irreps_out.append((l3, p3, mul))
                 paths.append((i_in, l2, len(irreps_out) - 1))
     return irreps_out, paths
+
+
+# --------------------------------------------------------------------------------------------
+# NEXT-1: radial network generating the weights (e3_oracle_next.c, readings R1-R4)
+# --------------------------------------------------------------------------------------------
+def poly_envelope(p, x):
+    """(u(x), du/dx) of the polynomial envelope (reading R2)."""
+    x = _f64(x).reshape(-1)
+    u, du = np.empty_like(x), np.empty_like(x)
+    _L().orc_poly_envelope(C.c_int(int(p)), C.c_int64(x.size), _p(x), _p(u), _p(du))
+    return u, du
+
+
+def radial_basis(K, p, rc, r):
+    """(f[n,K], df/dr[n,K]): Bessel basis times polynomial envelope (readings R1, R2)."""
+    r = _f64(r).reshape(-1)
+    f, d = np.empty((r.size, K)), np.empty((r.size, K))
+    _L().orc_radial_basis(C.c_int(int(K)), C.c_int(int(p)), C.c_double(float(rc)), C.c_int64(r.size), _p(r), _p(f), _p(d))
+    return f, d
+
+
+def radial_mlp_fwd(f, W1, W2, W3):
+    """w[n,M] = silu(silu(f W1) W2) W3 (reading R3)."""
+    f, W1, W2, W3 = _f64(f), _f64(W1), _f64(W2), _f64(W3)
+    n, K = f.shape
+    H, M = W3.shape
+    assert W1.shape == (K, H) and W2.shape == (H, H)
+    w = np.empty((n, M))
+    _L().orc_radial_mlp_fwd(C.c_int(K), C.c_int(H), C.c_int(M), C.c_int64(n), _p(f), _p(W1), _p(W2), _p(W3), _p(w))
+    return w
+
+
+def radial_mlp_bwd(f, W1, W2, W3, dw):
+    """(df, dW1, dW2, dW3) for a cotangent dw[n,M]."""
+    f, W1, W2, W3, dw = _f64(f), _f64(W1), _f64(W2), _f64(W3), _f64(dw)
+    n, K = f.shape
+    H, M = W3.shape
+    df, dW1, dW2, dW3 = np.empty((n, K)), np.empty((K, H)), np.empty((H, H)), np.empty((H, M))
+    _L().orc_radial_mlp_bwd(C.c_int(K), C.c_int(H), C.c_int(M), C.c_int64(n), _p(f), _p(W1), _p(W2), _p(W3), _p(dw),
+                            _p(df), _p(dW1), _p(dW2), _p(dW3))
+    return df, dW1, dW2, dW3
+
+
+def radial_weights(vec, K, p, rc, W1, W2, W3):
+    """w[E, P*C] generated from the edge vectors (R1-R4)."""
+    r = np.sqrt((_f64(vec).reshape(-1, 3) ** 2).sum(1))
+    f, _ = radial_basis(K, p, rc, r)
+    return radial_mlp_fwd(f, W1, W2, W3)
+
+
+def radial_weights_bwd(vec, K, p, rc, W1, W2, W3, dw):
+    """(grad_vec_radial[E,3], dW1, dW2, dW3): VJP of radial_weights; grad_vec = dE/dr * vec/|vec| (0 for a zero vector)."""
+    vec = _f64(vec).reshape(-1, 3)
+    r = np.sqrt((vec ** 2).sum(1))
+    f, dfdr = radial_basis(K, p, rc, r)
+    df, dW1, dW2, dW3 = radial_mlp_bwd(f, W1, W2, W3, dw)
+    dr = (df * dfdr).sum(1)
+    rhat = np.where(r[:, None] > 0, vec / np.where(r > 0, r, 1.0)[:, None], 0.0)
+    return dr[:, None] * rhat, dW1, dW2, dW3
