@@ -202,6 +202,36 @@ int e3_session_run_host(e3_session *session, const float *vec_h, const void *fea
                         const float *grad_out_h, float *out_h, float *grad_feats_h, void *grad_weights_h,
                         float *grad_vec_h, float *forces_h, int64_t *bytes_h2d, int64_t *bytes_d2h);
 
+/* ---------------------------------------------------------------------------------------------
+ * NEXT-1: the radial network that GENERATES the weights.  PAPER.md L82 (fusing the message-passing
+ * kernel is the authors' open item), L487-L491 (NequIP: num_rbf 8, swish, 64 hidden, 2 layers, polynomial envelope),
+ * L539-L542 (MACE: num_rbf 16, polynomial envelope), L497 (5 A cutoff).  The paper prints no formula; readings R1-R4
+ * (DESIGN.md): with r = |vec_e|, x = r / cutoff,
+ *   f_k(r) = sqrt(2/cutoff) sin(k pi r / cutoff) / r * u(x),  k = 1..num_rbf,
+ *   u(x) = 1 - (p+1)(p+2)/2 x^p + p(p+2) x^(p+1) - p(p+1)/2 x^(p+2)  (x < 1; 0 beyond),  p = envelope_p,
+ *   w[e, :] = silu(silu(f W1) W2) W3,  silu(a) = a / (1 + exp(-a)),  W1[num_rbf, 64], W2[64, 64], W3[64, n_out], no biases,
+ * and n_out = P*C so that w is exactly the `weights` operand of e3_tp_scatter_fwd/bwd of an E3_F32 plan.
+ * The last layer (edges x 64 x n_out) runs on the tensor cores (tcgen05.mma kind::tf32, TMEM accumulators) as a 3xTF32
+ * split product, accurate to fp32 rounding; the small layers run in fp32 on the CUDA cores.
+ * e3_radial_create copies the (HOST, row-major, float) parameter matrices to the device and synchronises.
+ * Limits: n_hidden == 64, num_rbf <= 16, n_out % 8 == 0 (else E3_ERR_UNSUPPORTED).
+ * e3_radial_weights_fwd: weights[E, n_out] (float, device) from vec[E,3]; workspace >= e3_radial_workspace_bytes.
+ * e3_radial_weights_bwd: given grad_weights[E, n_out] (float; the grad_weights output of e3_tp_scatter_bwd), computes
+ *   dE/dr through the network and writes (accumulate == 0) or adds (accumulate != 0) dE/dr * vec/|vec| to grad_vec[E,3]
+ *   (zero for a zero-length vector): adding it to the e3_sh_bwd result gives the full dE/dvec, which e3_force_reduce turns
+ *   into forces.  Gradients with respect to W1, W2, W3 are not computed by this library.
+ * Pointers 16-byte aligned; launches on `stream` only; deterministic.
+ * -------------------------------------------------------------------------------------------*/
+typedef struct e3_radial e3_radial;
+int e3_radial_create(e3_radial **net, int num_rbf, int envelope_p, double cutoff, int n_hidden, int n_out,
+                     const float *W1_h, const float *W2_h, const float *W3_h);
+int e3_radial_destroy(e3_radial *net);
+size_t e3_radial_workspace_bytes(const e3_radial *net, int64_t n_edges);
+int e3_radial_weights_fwd(const e3_radial *net, const float *vec /*[E,3]*/, int64_t n_edges, float *weights /*[E,n_out]*/,
+                          void *workspace, size_t workspace_bytes, e3_stream stream);
+int e3_radial_weights_bwd(const e3_radial *net, const float *vec, int64_t n_edges, const float *grad_weights /*[E,n_out]*/,
+                          float *grad_vec /*[E,3]*/, int accumulate, void *workspace, size_t workspace_bytes, e3_stream stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -23,6 +23,7 @@ SYMBOLS = [
     "e3_plan_get_cg", "e3_plan_kernel_info", "e3_plan_work", "e3_jit_check", "e3_graph_workspace_bytes",
     "e3_graph_prepare", "e3_sh_fwd", "e3_sh_bwd", "e3_tp_scatter_fwd", "e3_bwd_workspace_bytes", "e3_tp_scatter_bwd",
     "e3_force_reduce", "e3_profile_set_mid_event", "e3_measure_fp32_peak", "e3_session_create", "e3_session_destroy", "e3_session_run_host",
+    "e3_radial_create", "e3_radial_destroy", "e3_radial_workspace_bytes", "e3_radial_weights_fwd", "e3_radial_weights_bwd",
 ]
 
 
@@ -56,6 +57,8 @@ def lib():
         L.e3_graph_workspace_bytes.argtypes = [C.c_int64, C.c_int32]
         L.e3_bwd_workspace_bytes.restype = C.c_size_t
         L.e3_bwd_workspace_bytes.argtypes = [C.c_void_p, C.c_int64, C.c_int32]
+        L.e3_radial_workspace_bytes.restype = C.c_size_t
+        L.e3_radial_workspace_bytes.argtypes = [C.c_void_p, C.c_int64]
         _lib = L
     return _lib
 
@@ -285,3 +288,51 @@ class Session:
             self.destroy()
         except Exception:
             pass
+
+
+class Radial:
+    """Owns an ``e3_radial*`` (NEXT-1: the radial network generating the weights).  W1/W2/W3 are host float32 arrays."""
+
+    def __init__(self, num_rbf, envelope_p, cutoff, W1, W2, W3):
+        import numpy as np
+        W1, W2, W3 = (np.ascontiguousarray(a, dtype=np.float32) for a in (W1, W2, W3))
+        self.num_rbf, self.n_hidden, self.n_out = int(num_rbf), int(W2.shape[0]), int(W3.shape[1])
+        assert W1.shape == (num_rbf, self.n_hidden) and W3.shape[0] == self.n_hidden
+        self.handle = C.c_void_p()
+        _check(lib().e3_radial_create(C.byref(self.handle), int(num_rbf), int(envelope_p), C.c_double(float(cutoff)), self.n_hidden,
+                                      self.n_out, W1.ctypes.data_as(C.c_void_p), W2.ctypes.data_as(C.c_void_p),
+                                      W3.ctypes.data_as(C.c_void_p)), "e3_radial_create")
+
+    def workspace(self, n_edges, device):
+        return torch.empty(lib().e3_radial_workspace_bytes(self.handle, C.c_int64(n_edges)), dtype=torch.uint8, device=device)
+
+    def destroy(self):
+        if self.handle:
+            lib().e3_radial_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def e3_radial_weights_fwd(net: Radial, vec, out=None, workspace=None, stream=None):
+    _dev(vec, torch.float32)
+    E = vec.shape[0]
+    w = out if out is not None else torch.empty((E, net.n_out), dtype=torch.float32, device=vec.device)
+    ws = workspace if workspace is not None else net.workspace(E, vec.device)
+    _check(lib().e3_radial_weights_fwd(net.handle, _ptr(vec), C.c_int64(E), _ptr(_dev(w, torch.float32)), _ptr(ws),
+                                       C.c_size_t(ws.numel()), _stream(stream)), "e3_radial_weights_fwd")
+    return w
+
+
+def e3_radial_weights_bwd(net: Radial, vec, grad_weights, grad_vec=None, accumulate=False, workspace=None, stream=None):
+    _dev(vec, torch.float32); _dev(grad_weights, torch.float32)
+    E = vec.shape[0]
+    gv = grad_vec if grad_vec is not None else torch.empty((E, 3), dtype=torch.float32, device=vec.device)
+    ws = workspace if workspace is not None else net.workspace(E, vec.device)
+    _check(lib().e3_radial_weights_bwd(net.handle, _ptr(vec), C.c_int64(E), _ptr(grad_weights), _ptr(_dev(gv, torch.float32)),
+                                       int(bool(accumulate)), _ptr(ws), C.c_size_t(ws.numel()), _stream(stream)), "e3_radial_weights_bwd")
+    return gv
