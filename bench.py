@@ -457,6 +457,57 @@ def measure_config(k, args, world, rank, local, dev, steps, want_cpu, want_e2e):
                               "how": "148 SM x 128 lanes x 2 x 1.965 GHz; measured = e3_measure_fp32_peak (FFMA2 chains in registers, 0.3 s)"},
                  "kernel_ms": kms, "kernel_info": {"fwd": plan.kernel_info(0), "bwd": plan.kernel_info(1)}}
 
+    # NEXT-1: the same step with the weights GENERATED on the device by the radial network (PAPER.md L487-L491,
+    # L539-L542) instead of being read as an input: radial fwd (hidden layers + tcgen05 3xTF32 GEMM) -> TP fwd -> TP VJP ->
+    # radial VJP (tcgen05 GEMM + hidden layers), reported beside the given-weights numbers (fp32 plans only)
+    if rank == 0 and args.radial and cfg.storage == "f32":
+        K_rbf = 16 if cfg.sh_lmax >= 3 else 8
+        nrng = np.random.Generator(np.random.Philox(cfg.seed + 3000))
+        W1 = (nrng.normal(size=(K_rbf, 64)) / np.sqrt(K_rbf)).astype(np.float32)
+        W2 = (nrng.normal(size=(64, 64)) / 8.0).astype(np.float32)
+        W3 = (nrng.normal(size=(64, P * C)) / 8.0 * W.w_sigma(cfg, P)).astype(np.float32)
+        net = B.Radial(K_rbf, 6, 5.0, W1, W2, W3)
+        rws = net.workspace(E, dev)
+        evs = {}
+
+        def rstep(record):
+            def mark(name):
+                if record:
+                    e_ = torch.cuda.Event(enable_timing=True); e_.record(stream); evs.setdefault(name, []).append(e_)
+            mark("t0")
+            B.e3_radial_weights_fwd(net, vec, out=w, workspace=rws)
+            mark("radial_fwd")
+            chk(L.e3_tp_scatter_fwd(plan.handle, p(x), p(sh), p(w), p(snd), p(rcv), p(row_ptr), Ct.c_int64(E), Ct.c_int32(N), p(out), sp), "fwd")
+            mark("tp_fwd")
+            chk(L.e3_tp_scatter_bwd(plan.handle, p(x), p(sh), p(w), p(snd), p(rcv), p(row_ptr), p(perm_s), p(col_ptr), Ct.c_int64(E), Ct.c_int32(N),
+                                    p(G), p(gfe), p(gsh), p(gw), p(ws), Ct.c_size_t(ws.numel()), sp), "bwd")
+            mark("tp_bwd")
+            chk(L.e3_sh_bwd(plan.handle, p(vec), p(gsh), Ct.c_int64(E), p(gvec), sp), "sh_bwd")
+            B.e3_radial_weights_bwd(net, vec, gw, grad_vec=gvec, accumulate=True, workspace=rws)
+            mark("radial_bwd")
+        for _ in range(3):
+            rstep(False)
+        nr = max(3, min(steps, 20))
+        for _ in range(nr):
+            rstep(True)
+        torch.cuda.synchronize()
+        names = ["t0", "radial_fwd", "tp_fwd", "tp_bwd", "radial_bwd"]
+        rms = {b_: float(np.mean([evs[a_][i].elapsed_time(evs[b_][i]) for i in range(nr)])) for a_, b_ in zip(names[:-1], names[1:])}
+        gemm_flop = 2.0 * E * 64 * P * C
+        w_bytes = E * P * C * 4
+        block["radial"] = {
+            "what": "weights generated by the radial network (num_rbf %d, polynomial envelope p=6, 64-64 silu, last layer on tcgen05 3xTF32); not fused into the TP kernels: w is written once and read back" % K_rbf,
+            "ms": rms, "ms_fwd_plus_vjp_generated": sum(rms.values()),
+            "edges_per_s_fwd_plus_vjp_generated": E / (sum(rms.values()) * 1e-3),
+            "last_layer": {"algorithmic_flops": gemm_flop, "tflops_fwd": gemm_flop / (rms["radial_fwd"] * 1e-3) / 1e12,
+                           "bytes_written_fwd": w_bytes, "write_GBps_fwd": w_bytes / (rms["radial_fwd"] * 1e-3) / 1e9,
+                           "frac_of_hbm_fwd": w_bytes / (rms["radial_fwd"] * 1e-3) / 1e9 / hbm_peak,
+                           "bytes_read_bwd": w_bytes, "read_GBps_bwd": w_bytes / (rms["radial_bwd"] * 1e-3) / 1e9,
+                           "frac_of_hbm_bwd": w_bytes / (rms["radial_bwd"] * 1e-3) / 1e9 / hbm_peak,
+                           "bound": "hbm (the un-fused product writes / re-reads E x P*C x 4 bytes; the MMA work, 3 x 2*E*64*P*C flop of TF32, is < 10 % of the tensor peak)"}}
+        net.destroy()
+        del rws
+
     # free the device-resident run before the host-buffer one (config 4 holds ~125 GB)
     del out, sh, gfe, gsh, gw, gvec, F, ws, gws, row_ptr, col_ptr, perm_s
     gc.collect()
@@ -539,8 +590,8 @@ def run_ours(args):
                 "ms_per_step": blk["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": blk["dtype"], "data": "synthetic"}
         for key in ("config", "clocks", "gpu_launches", "e2e", "roofline", "roofline_fwd", "tp_fwd_plus_vjp", "alu_peak", "kernel_ms",
-                    "kernel_info", "cpu_baseline"):
-            line[key] = blk[key]
+                    "kernel_info", "cpu_baseline", "radial"):
+            line[key] = blk.get(key)
         line["csrc_sha"] = kernel_sources_sha()
         if sec is not None:
             sec["metric"] = METRIC
@@ -559,6 +610,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-secondary", action="store_true")
+    ap.add_argument("--no-radial", dest="radial", action="store_false", help="skip the NEXT-1 block (generated weights)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -20,6 +20,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -76,107 +77,116 @@ __device__ __forceinline__ void radial_feature(int k, float r, float rc, int p, 
     dfdr = db * u + b * du / rc;
 }
 
-// one warp per edge (grid-stride); lane owns hidden units `lane` and `lane + 32`
+// Hidden layers, forward and (BWD) their VJP.  A warp processes FOUR edges per pass; a lane owns hidden units `lane` and
+// `lane + 32` of all four.  The activations of the previous layer sit transposed in a per-warp shared-memory buffer [unit][edge], so
+// one broadcast 16-byte load serves eight FMAs (two units x four edges) beside the two weight loads: 3 LDS per 8 FMA instead of the
+// 2 LDS + 2 SHFL per 2 FMA of a one-edge-per-warp loop (which ran at 87 % of the LSU pipe, profiles/r02_radial.md).
+template <bool BWD>
 __global__ void __launch_bounds__(128) radial_hidden_kernel(const float *__restrict__ vec, long long E, int K, int p, float rc,
-                                                            const float *__restrict__ W1, const float *__restrict__ W2, float *__restrict__ h2out)
+                                                            const float *__restrict__ W1, const float *__restrict__ W2, const float *__restrict__ W2T,
+                                                            float *__restrict__ h2out, const float *__restrict__ dh2, float *__restrict__ gvec, int accumulate)
 {
-    __shared__ float W1s[kMaxRbf * kH];
-    __shared__ float W2s[kH * kH];
-    for (int i = threadIdx.x; i < K * kH; i += blockDim.x) W1s[i] = W1[i];
-    for (int i = threadIdx.x; i < kH * kH; i += blockDim.x) W2s[i] = W2[i];
+    extern __shared__ __align__(16) float hsm[];
+    float *W1s = hsm;                                   // [K][64]
+    float *W2s = W1s + kMaxRbf * kH;                    // [64][64]
+    float *W2Ts = W2s + kH * kH;                        // [64][64] transposed (BWD only)
+    float *W1Ts = W2Ts + (BWD ? kH * kH : 0);           // [64][16] transposed (BWD only)
+    float *wbuf = W1Ts + (BWD ? kH * kMaxRbf : 0);      // per warp: act[64][4] + feat[16][4] + dfeat[16][4]
+    for (int i = threadIdx.x; i < kMaxRbf * kH; i += blockDim.x) W1s[i] = i < K * kH ? W1[i] : 0.0f;
+    for (int i = threadIdx.x; i < kH * kH; i += blockDim.x) { W2s[i] = W2[i]; if (BWD) W2Ts[i] = W2T[i]; }
+    if (BWD) for (int i = threadIdx.x; i < kH * kMaxRbf; i += blockDim.x) { const int u = i / kMaxRbf, k = i % kMaxRbf; W1Ts[i] = k < K ? W1[k * kH + u] : 0.0f; }
     __syncthreads();
-    const int lane = threadIdx.x & 31;
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    float *act = wbuf + wib * (kH * 4 + 2 * kMaxRbf * 4), *feat = act + kH * 4, *dfeat = feat + kMaxRbf * 4;
     const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
-    for (long long e = warp; e < E; e += nwarps) {
-        const float vx = vec[3 * e], vy = vec[3 * e + 1], vz = vec[3 * e + 2];
+    const int el = lane >> 3, kk = lane & 7;            // this lane evaluates radial features kk and kk + 8 of edge el
+    for (long long e0 = warp * 4; e0 < E; e0 += nwarps * 4) {
+        const long long em = e0 + el < E ? e0 + el : E - 1;
+        const float vx = vec[3 * em], vy = vec[3 * em + 1], vz = vec[3 * em + 2];
         const float r = sqrtf(vx * vx + vy * vy + vz * vz);
-        float f = 0.0f, dd;
-        if (lane < K) radial_feature(lane, r, rc, p, f, dd);
-        float a0 = 0.0f, a1 = 0.0f;
+        float f0 = 0.0f, f1 = 0.0f, d0 = 0.0f, d1 = 0.0f;
+        if (kk < K) radial_feature(kk, r, rc, p, f0, d0);
+        if (kk + 8 < K) radial_feature(kk + 8, r, rc, p, f1, d1);
+        __syncwarp();
+        feat[kk * 4 + el] = f0; feat[(kk + 8) * 4 + el] = f1;
+        __syncwarp();
+        float a1[2][4] = {};
         for (int k = 0; k < K; ++k) {
-            const float fk = __shfl_sync(0xffffffffu, f, k);
-            a0 = fmaf(fk, W1s[k * kH + lane], a0);
-            a1 = fmaf(fk, W1s[k * kH + lane + 32], a1);
+            const float4 fk = *reinterpret_cast<const float4 *>(feat + k * 4);
+            const float w0 = W1s[k * kH + lane], w1 = W1s[k * kH + lane + 32];
+            a1[0][0] = fmaf(fk.x, w0, a1[0][0]); a1[0][1] = fmaf(fk.y, w0, a1[0][1]); a1[0][2] = fmaf(fk.z, w0, a1[0][2]); a1[0][3] = fmaf(fk.w, w0, a1[0][3]);
+            a1[1][0] = fmaf(fk.x, w1, a1[1][0]); a1[1][1] = fmaf(fk.y, w1, a1[1][1]); a1[1][2] = fmaf(fk.z, w1, a1[1][2]); a1[1][3] = fmaf(fk.w, w1, a1[1][3]);
         }
-        const float h0 = silu_f(a0), h1 = silu_f(a1);
-        float b0 = 0.0f, b1 = 0.0f;
+        *reinterpret_cast<float4 *>(act + lane * 4) = make_float4(silu_f(a1[0][0]), silu_f(a1[0][1]), silu_f(a1[0][2]), silu_f(a1[0][3]));
+        *reinterpret_cast<float4 *>(act + (lane + 32) * 4) = make_float4(silu_f(a1[1][0]), silu_f(a1[1][1]), silu_f(a1[1][2]), silu_f(a1[1][3]));
+        __syncwarp();
+        float a2[2][4] = {};
 #pragma unroll 8
-        for (int i = 0; i < 32; ++i) {
-            const float hi0 = __shfl_sync(0xffffffffu, h0, i), hi1 = __shfl_sync(0xffffffffu, h1, i);
-            b0 = fmaf(hi0, W2s[i * kH + lane], b0);
-            b1 = fmaf(hi0, W2s[i * kH + lane + 32], b1);
-            b0 = fmaf(hi1, W2s[(i + 32) * kH + lane], b0);
-            b1 = fmaf(hi1, W2s[(i + 32) * kH + lane + 32], b1);
+        for (int i = 0; i < kH; ++i) {
+            const float4 h = *reinterpret_cast<const float4 *>(act + i * 4);
+            const float w0 = W2s[i * kH + lane], w1 = W2s[i * kH + lane + 32];
+            a2[0][0] = fmaf(h.x, w0, a2[0][0]); a2[0][1] = fmaf(h.y, w0, a2[0][1]); a2[0][2] = fmaf(h.z, w0, a2[0][2]); a2[0][3] = fmaf(h.w, w0, a2[0][3]);
+            a2[1][0] = fmaf(h.x, w1, a2[1][0]); a2[1][1] = fmaf(h.y, w1, a2[1][1]); a2[1][2] = fmaf(h.z, w1, a2[1][2]); a2[1][3] = fmaf(h.w, w1, a2[1][3]);
         }
-        h2out[e * kH + lane] = silu_f(b0);
-        h2out[e * kH + lane + 32] = silu_f(b1);
-    }
-}
-
-// backward of the hidden layers: dh2[E,64] -> d r -> grad_vec (+)= dE/dr * vec/|vec|
-__global__ void __launch_bounds__(128) radial_hidden_bwd_kernel(const float *__restrict__ vec, long long E, int K, int p, float rc,
-                                                                const float *__restrict__ W1, const float *__restrict__ W2, const float *__restrict__ W2T,
-                                                                const float *__restrict__ dh2, float *__restrict__ gvec, int accumulate)
-{
-    __shared__ float W1s[kMaxRbf * kH];
-    __shared__ float W2s[kH * kH];
-    __shared__ float W2Ts[kH * kH];
-    for (int i = threadIdx.x; i < K * kH; i += blockDim.x) W1s[i] = W1[i];
-    for (int i = threadIdx.x; i < kH * kH; i += blockDim.x) { W2s[i] = W2[i]; W2Ts[i] = W2T[i]; }
-    __syncthreads();
-    const int lane = threadIdx.x & 31;
-    const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
-    for (long long e = warp; e < E; e += nwarps) {
-        const float vx = vec[3 * e], vy = vec[3 * e + 1], vz = vec[3 * e + 2];
-        const float r = sqrtf(vx * vx + vy * vy + vz * vz);
-        float f = 0.0f, dfdr = 0.0f;
-        if (lane < K) radial_feature(lane, r, rc, p, f, dfdr);
-        float a0 = 0.0f, a1 = 0.0f;
-        for (int k = 0; k < K; ++k) {
-            const float fk = __shfl_sync(0xffffffffu, f, k);
-            a0 = fmaf(fk, W1s[k * kH + lane], a0);
-            a1 = fmaf(fk, W1s[k * kH + lane + 32], a1);
-        }
-        const float h0 = silu_f(a0), h1 = silu_f(a1);
-        float b0 = 0.0f, b1 = 0.0f;
-#pragma unroll 8
-        for (int i = 0; i < 32; ++i) {
-            const float hi0 = __shfl_sync(0xffffffffu, h0, i), hi1 = __shfl_sync(0xffffffffu, h1, i);
-            b0 = fmaf(hi0, W2s[i * kH + lane], b0);
-            b1 = fmaf(hi0, W2s[i * kH + lane + 32], b1);
-            b0 = fmaf(hi1, W2s[(i + 32) * kH + lane], b0);
-            b1 = fmaf(hi1, W2s[(i + 32) * kH + lane + 32], b1);
-        }
-        // dL/da2 for units lane, lane + 32
-        const float g20 = dh2[e * kH + lane] * dsilu_f(b0), g21 = dh2[e * kH + lane + 32] * dsilu_f(b1);
-        // dL/dh1[i] = sum_j g2[j] W2[i][j]  (W2T[j][i] read contiguously over the lanes)
-        float t0 = 0.0f, t1 = 0.0f;
-#pragma unroll 8
-        for (int j = 0; j < 32; ++j) {
-            const float gj0 = __shfl_sync(0xffffffffu, g20, j), gj1 = __shfl_sync(0xffffffffu, g21, j);
-            t0 = fmaf(gj0, W2Ts[j * kH + lane], t0);
-            t1 = fmaf(gj0, W2Ts[j * kH + lane + 32], t1);
-            t0 = fmaf(gj1, W2Ts[(j + 32) * kH + lane], t0);
-            t1 = fmaf(gj1, W2Ts[(j + 32) * kH + lane + 32], t1);
-        }
-        const float g10 = t0 * dsilu_f(a0), g11 = t1 * dsilu_f(a1);
-        // d f_k = sum_i g1[i] W1[k][i]; dr = sum_k d f_k * d f_k / d r   (fixed-order butterflies: deterministic)
-        float dr = 0.0f;
-        for (int k = 0; k < K; ++k) {
-            float part = g10 * W1s[k * kH + lane] + g11 * W1s[k * kH + lane + 32];
+        if (!BWD) {
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
-            const float dk = __shfl_sync(0xffffffffu, dfdr, k);
-            dr = fmaf(part, dk, dr);
+            for (int q = 0; q < 4; ++q)
+                if (e0 + q < E) {      // h2 split into its TF32 high part and the exact remainder: the B operand of the output-layer GEMM
+                    const float v0 = silu_f(a2[0][q]), v1 = silu_f(a2[1][q]);
+                    const float h0 = __uint_as_float(__float_as_uint(v0) & 0xffffe000u), h1 = __uint_as_float(__float_as_uint(v1) & 0xffffe000u);
+                    h2out[(e0 + q) * kH + lane] = h0; h2out[(e0 + q) * kH + lane + 32] = h1;
+                    h2out[(E + e0 + q) * kH + lane] = v0 - h0; h2out[(E + e0 + q) * kH + lane + 32] = v1 - h1;
+                }
+            continue;
         }
-        if (lane == 0) {
+        // ---- VJP: dL/da2 -> dL/dh1 -> dL/da1 -> d f -> d r
+        float g2[2][4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const long long eq = e0 + q < E ? e0 + q : E - 1;
+            g2[0][q] = dh2[eq * kH + lane] * dsilu_f(a2[0][q]);
+            g2[1][q] = dh2[eq * kH + lane + 32] * dsilu_f(a2[1][q]);
+        }
+        __syncwarp();
+        *reinterpret_cast<float4 *>(act + lane * 4) = make_float4(g2[0][0], g2[0][1], g2[0][2], g2[0][3]);
+        *reinterpret_cast<float4 *>(act + (lane + 32) * 4) = make_float4(g2[1][0], g2[1][1], g2[1][2], g2[1][3]);
+        __syncwarp();
+        float t[2][4] = {};
+#pragma unroll 8
+        for (int j = 0; j < kH; ++j) {                   // dL/dh1[i] = sum_j g2[j] W2[i][j]; W2T[j][i] is contiguous over the lanes
+            const float4 g = *reinterpret_cast<const float4 *>(act + j * 4);
+            const float w0 = W2Ts[j * kH + lane], w1 = W2Ts[j * kH + lane + 32];
+            t[0][0] = fmaf(g.x, w0, t[0][0]); t[0][1] = fmaf(g.y, w0, t[0][1]); t[0][2] = fmaf(g.z, w0, t[0][2]); t[0][3] = fmaf(g.w, w0, t[0][3]);
+            t[1][0] = fmaf(g.x, w1, t[1][0]); t[1][1] = fmaf(g.y, w1, t[1][1]); t[1][2] = fmaf(g.z, w1, t[1][2]); t[1][3] = fmaf(g.w, w1, t[1][3]);
+        }
+        __syncwarp();
+        *reinterpret_cast<float4 *>(act + lane * 4) = make_float4(t[0][0] * dsilu_f(a1[0][0]), t[0][1] * dsilu_f(a1[0][1]), t[0][2] * dsilu_f(a1[0][2]), t[0][3] * dsilu_f(a1[0][3]));
+        *reinterpret_cast<float4 *>(act + (lane + 32) * 4) = make_float4(t[1][0] * dsilu_f(a1[1][0]), t[1][1] * dsilu_f(a1[1][1]), t[1][2] * dsilu_f(a1[1][2]), t[1][3] * dsilu_f(a1[1][3]));
+        __syncwarp();
+        float df0 = 0.0f, df1 = 0.0f;                    // d f_k of edge el for k = kk, kk + 8: sum over the 64 units in ascending order
+#pragma unroll 8
+        for (int i = 0; i < kH; ++i) {
+            const float g = act[i * 4 + el];
+            df0 = fmaf(g, W1Ts[i * kMaxRbf + kk], df0);
+            df1 = fmaf(g, W1Ts[i * kMaxRbf + kk + 8], df1);
+        }
+        float dr = df0 * d0 + df1 * d1;
+        dr += __shfl_xor_sync(0xffffffffu, dr, 1);
+        dr += __shfl_xor_sync(0xffffffffu, dr, 2);
+        dr += __shfl_xor_sync(0xffffffffu, dr, 4);
+        if (kk == 0 && e0 + el < E) {
+            const long long e = e0 + el;
             const float inv = r > 0.0f ? 1.0f / r : 0.0f;
             const float gx = dr * vx * inv, gy = dr * vy * inv, gz = dr * vz * inv;
             if (accumulate) { gvec[3 * e] += gx; gvec[3 * e + 1] += gy; gvec[3 * e + 2] += gz; }
             else { gvec[3 * e] = gx; gvec[3 * e + 1] = gy; gvec[3 * e + 2] = gz; }
         }
+        (void)dfeat;
     }
 }
+
+constexpr int kHiddenSmemFwd = (kMaxRbf * kH + kH * kH + 4 * (kH * 4 + 2 * kMaxRbf * 4)) * 4;
+constexpr int kHiddenSmemBwd = (kMaxRbf * kH + 2 * kH * kH + kH * kMaxRbf + 4 * (kH * 4 + 2 * kMaxRbf * 4)) * 4;
 
 // split W3 into TF32 high / low parts, both as [64][n_out] and transposed [n_out][64]
 __global__ void radial_split_w3_kernel(const float *__restrict__ W3, int n_out, float *__restrict__ hi, float *__restrict__ lo,
@@ -215,99 +225,166 @@ __device__ __forceinline__ uint32_t canon_off(int row, int k)    // byte offset 
     return (uint32_t)((row >> 3) * 2048 + (k >> 2) * 128 + (row & 7) * 16 + (k & 3) * 4);
 }
 
-__global__ void __launch_bounds__(128, 2) radial_gemm_kernel(const float *__restrict__ A, long long lda, const float *__restrict__ Bhi,
-                                                             const float *__restrict__ Blo, long long ldb, float *__restrict__ D, long long ldd,
-                                                             long long M, int N, int n_tiles, int k_chunks, long long Kt)
+__device__ __forceinline__ float tf32_hi(float v) { return __uint_as_float(__float_as_uint(v) & 0xffffe000u); }
+
+__device__ __forceinline__ void mbar_wait_parity(uint32_t bar, uint32_t parity)
 {
+    asm volatile("{\n.reg .pred p;\nLAB_WAIT:\nmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra DONE;\nbra LAB_WAIT;\nDONE:\n}"
+                 :: "r"(bar), "r"(parity) : "memory");
+}
+
+// the three products of one K chunk (64 = 8 MMA steps of K = 8): lo*hi, hi*lo, hi*hi, smallest terms first
+__device__ __forceinline__ void issue_chunk(uint32_t tmem_d, uint32_t sAhi, uint32_t sAlo, uint32_t sBhi, uint32_t sBlo, uint32_t idesc, bool first, int nprod = 3)
+{
+    if (nprod == 1) {           // measurement aid (E3_RADIAL_PRODUCTS=1): plain TF32, hi*hi only -- NOT fp32 accurate
+#pragma unroll
+        for (int ks = 0; ks < kTileK / 8; ++ks) {
+            const uint64_t ahi = umma_desc(sAhi + ks * 256), bhi = umma_desc(sBhi + ks * 256);
+            const uint32_t acc0 = (!first || ks > 0) ? 1u : 0u;
+            asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}"
+                         :: "r"(tmem_d), "l"(ahi), "l"(bhi), "r"(idesc), "r"(acc0) : "memory");
+        }
+        return;
+    }
+#pragma unroll
+    for (int ks = 0; ks < kTileK / 8; ++ks) {       // one MMA covers K = 8 (32 bytes = two core matrices): advance 256 bytes
+        const uint64_t ahi = umma_desc(sAhi + ks * 256), alo = umma_desc(sAlo + ks * 256);
+        const uint64_t bhi = umma_desc(sBhi + ks * 256), blo = umma_desc(sBlo + ks * 256);
+        const uint32_t acc0 = (!first || ks > 0) ? 1u : 0u;
+        asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}"
+                     :: "r"(tmem_d), "l"(alo), "l"(bhi), "r"(idesc), "r"(acc0) : "memory");
+        asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}"
+                     :: "r"(tmem_d), "l"(ahi), "l"(blo), "r"(idesc), "r"(1u) : "memory");
+        asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}"
+                     :: "r"(tmem_d), "l"(ahi), "l"(bhi), "r"(idesc), "r"(1u) : "memory");
+    }
+}
+
+// TMEM -> registers -> shared-memory transpose -> global: warp w owns TMEM lanes 32 w .. 32 w + 31 (= tile rows).  A thread holds 32
+// consecutive columns of ITS row; written out directly that is 16 bytes per lane at a row stride (half-filled sectors).  Each
+// 32 x 32 block therefore goes through a per-warp staging buffer (row stride 36 floats: conflict-free both ways) and leaves as
+// four full 128-byte row segments per store instruction.
+template <int NT>
+__device__ __forceinline__ void epilogue_tile(uint32_t tmem_d, int warp8, int lane, float *__restrict__ stg, float *__restrict__ D, long long ldd,
+                                              long long m0, long long M, int n0, int N)
+{
+    // eight warps: warp8 % 4 selects the TMEM lane quarter (tile rows 32 q .. 32 q + 31), warp8 / 4 the column half
+    const int warp = warp8 & 3;
+    float *sw = stg + warp8 * (32 * 36);
+#pragma unroll 1
+    for (int c0 = (warp8 >> 2) * (NT / 2); c0 < (warp8 >> 2) * (NT / 2) + NT / 2; c0 += 32) {
+        uint32_t v[32];
+        const uint32_t taddr = tmem_d + ((uint32_t)(warp * 32) << 16) + (uint32_t)c0;
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+                     "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+                     "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+                     : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
+                       "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]),
+                       "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]),
+                       "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+                     : "r"(taddr) : "memory");
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        __syncwarp();
+#pragma unroll
+        for (int j = 0; j < 32; j += 4)
+            *reinterpret_cast<float4 *>(sw + lane * 36 + j) = make_float4(__uint_as_float(v[j]), __uint_as_float(v[j + 1]), __uint_as_float(v[j + 2]), __uint_as_float(v[j + 3]));
+        __syncwarp();
+        const int col = n0 + c0 + 4 * (lane & 7);
+#pragma unroll
+        for (int it = 0; it < 8; ++it) {
+            const int rl = it * 4 + (lane >> 3);
+            const long long row = m0 + warp * 32 + rl;
+            const float4 o = *reinterpret_cast<const float4 *>(sw + rl * 36 + 4 * (lane & 7));
+            if (row < M) {
+                float *dp = D + row * ldd + col;
+                if (col + 4 <= N && (ldd & 3) == 0) __stcs(reinterpret_cast<float4 *>(dp), o);
+                else {
+                    if (col < N) dp[0] = o.x;
+                    if (col + 1 < N) dp[1] = o.y;
+                    if (col + 2 < N) dp[2] = o.z;
+                    if (col + 3 < N) dp[3] = o.w;
+                }
+            }
+        }
+    }
+}
+
+// thread -> (row, 16-byte quad) of a [rows x 64] fp32 operand tile for pass j: a warp covers 8 consecutive rows x 4 consecutive quads,
+// i.e. 64 contiguous bytes of 8 rows in global memory (whole sectors) and 512 contiguous bytes in the canonical shared-memory layout
+// (conflict-free).  Eight warps: row = 16 j + 8 (warp / 4) + (lane & 7), quad = 4 (warp % 4) + (lane >> 3)
+#define TILE_ROW(j) ((j) * 16 + (warp >> 2) * 8 + (lane & 7))
+#define TILE_QUAD() ((warp & 3) * 4 + (lane >> 3))
+
+// FORWARD, features as the M dimension:  D[f, e] = sum_k W3T[n_base + f, k] * h2[e, k]  for a slab of 128 output features (A operand,
+// staged once per CTA) and a run of 128-edge tiles (B operand = the rows of h2, already split into TF32 high / low parts by the hidden
+// kernel, brought in by 16-byte cp.async straight into the canonical layout, double-buffered).  In TMEM a lane is a FEATURE and a
+// column an EDGE, so a tcgen05.ld leaves every warp with 32 consecutive features of one edge per register: each store instruction
+// writes one full 128-byte line of w[e, n_base + 32 q ..] -- no shared-memory transpose.  While the eight warps drain tile i - 1, the
+// tensor core computes tile i (second TMEM buffer) and the copies of tile i + 1 are in flight.
+__global__ void __launch_bounds__(256, 1) radial_gemm_fwd_kernel(const float *__restrict__ Hhi, const float *__restrict__ Hlo, const float *__restrict__ W3Thi,
+                                                                 const float *__restrict__ W3Tlo, float *__restrict__ D, long long ldd, long long E, int N,
+                                                                 int tiles_per_cta, int nprod)
+{
+    constexpr int NT = 128;                                                  // edges per tile (MMA N)
     extern __shared__ __align__(1024) unsigned char smem[];
-    unsigned char *sAhi = smem, *sAlo = smem + 32768, *sBhi = smem + 65536, *sBlo = smem + 65536 + 16384;
-    __shared__ __align__(8) unsigned long long mbar;
+    unsigned char *sAhi = smem, *sAlo = smem + 32768;                       // the feature slab [128 x 64], high / low
+    unsigned char *sB = smem + 65536;                                       // 2 buffers x (hi 32 KB, lo 32 KB)
+    __shared__ __align__(8) unsigned long long mbar[2];
     __shared__ uint32_t tmem_base_s;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const long long m0 = (long long)blockIdx.x * kTileM;
-    const uint32_t mbar_s = (uint32_t)__cvta_generic_to_shared(&mbar);
+    const int n_base = blockIdx.x * kTileM;
+    const long long n_etiles = (E + NT - 1) / NT;
+    const long long t_begin = (long long)blockIdx.y * tiles_per_cta;
+    const long long t_end = t_begin + tiles_per_cta < n_etiles ? t_begin + tiles_per_cta : n_etiles;
+    if (t_begin >= t_end) return;
+    const uint32_t mbar_s = (uint32_t)__cvta_generic_to_shared(&mbar[0]);
     if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 64;" :: "r"((uint32_t)__cvta_generic_to_shared(&tmem_base_s)) : "memory");
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 256;" :: "r"((uint32_t)__cvta_generic_to_shared(&tmem_base_s)) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     if (tid == 0) {
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(mbar_s) : "memory");
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(mbar_s + 8) : "memory");
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    const uint32_t sAhi_s = (uint32_t)__cvta_generic_to_shared(sAhi), sAlo_s = sAhi_s + 32768, sB_s = sAhi_s + 65536;
+    // stationary operand: 128 rows of W3^T (zero beyond N), high and low parts
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        const int row = TILE_ROW(j), q = TILE_QUAD();
+        const uint32_t off = canon_off(row, q * 4);
+        const bool v = n_base + row < N;
+        const float *sh_ = W3Thi + (long long)(v ? n_base + row : 0) * kH + q * 4, *sl_ = W3Tlo + (long long)(v ? n_base + row : 0) * kH + q * 4;
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(sAhi_s + off), "l"(sh_), "r"(v ? 16 : 0) : "memory");
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(sAlo_s + off), "l"(sl_), "r"(v ? 16 : 0) : "memory");
+    }
+    auto issue_b = [&](long long t, int buf) {
+        const long long e0 = t * NT;
+        const uint32_t bh = sB_s + buf * 65536, bl = bh + 32768;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const int row = TILE_ROW(j), q = TILE_QUAD();
+            const uint32_t off = canon_off(row, q * 4);
+            const bool v = e0 + row < E;
+            const long long er = v ? e0 + row : 0;
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(bh + off), "l"(Hhi + er * kH + q * 4), "r"(v ? 16 : 0) : "memory");
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(bl + off), "l"(Hlo + er * kH + q * 4), "r"(v ? 16 : 0) : "memory");
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    issue_b(t_begin, 0);
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem = tmem_base_s;
-    // instruction descriptor: D fp32, A/B TF32, both K-major, N = 64, M = 128
-    const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(kTileN >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
-    const uint32_t sAhi_s = (uint32_t)__cvta_generic_to_shared(sAhi), sAlo_s = (uint32_t)__cvta_generic_to_shared(sAlo);
-    const uint32_t sBhi_s = (uint32_t)__cvta_generic_to_shared(sBhi), sBlo_s = (uint32_t)__cvta_generic_to_shared(sBlo);
-    uint32_t phase = 0;
-    for (int nt = 0; nt < n_tiles; ++nt) {
-        const int n0 = nt * kTileN;
-        for (int kc = 0; kc < k_chunks; ++kc) {
-            const long long k0 = (long long)kc * kTileK;
-            // A chunk [128 x 64]: 2048 float4; thread t takes float4 (row = i / 16, quad = i % 16); a float4 is one core-matrix row
-            if (nt == 0 || k_chunks > 1) {
-                for (int i = tid; i < kTileM * 16; i += 128) {
-                    const int row = i >> 4, q = i & 15;
-                    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-                    if (m0 + row < M && k0 + q * 4 + 4 <= Kt) v = *reinterpret_cast<const float4 *>(A + (m0 + row) * lda + k0 + q * 4);
-                    float4 h, l;
-                    h.x = __uint_as_float(__float_as_uint(v.x) & 0xffffe000u); l.x = v.x - h.x;
-                    h.y = __uint_as_float(__float_as_uint(v.y) & 0xffffe000u); l.y = v.y - h.y;
-                    h.z = __uint_as_float(__float_as_uint(v.z) & 0xffffe000u); l.z = v.z - h.z;
-                    h.w = __uint_as_float(__float_as_uint(v.w) & 0xffffe000u); l.w = v.w - h.w;
-                    const uint32_t off = canon_off(row, q * 4);
-                    *reinterpret_cast<float4 *>(sAhi + off) = h;
-                    *reinterpret_cast<float4 *>(sAlo + off) = l;
-                }
-            }
-            // B chunk [64 x 64] (rows = output columns n0 + row, or zero beyond N)
-            for (int i = tid; i < kTileN * 16; i += 128) {
-                const int row = i >> 4, q = i & 15;
-                float4 h = make_float4(0.f, 0.f, 0.f, 0.f), l = h;
-                if (n0 + row < N && k0 + q * 4 + 4 <= Kt) {
-                    h = *reinterpret_cast<const float4 *>(Bhi + (long long)(n0 + row) * ldb + k0 + q * 4);
-                    l = *reinterpret_cast<const float4 *>(Blo + (long long)(n0 + row) * ldb + k0 + q * 4);
-                }
-                const uint32_t off = canon_off(row, q * 4);
-                *reinterpret_cast<float4 *>(sBhi + off) = h;
-                *reinterpret_cast<float4 *>(sBlo + off) = l;
-            }
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");       // generic-proxy stores -> visible to the tensor core (async proxy)
-            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-            __syncthreads();
-            if (tid == 0) {
-                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-#pragma unroll
-                for (int ks = 0; ks < kTileK / 8; ++ks) {       // one MMA covers K = 8 (32 bytes = two core matrices): advance 256 bytes
-                    const uint64_t ahi = umma_desc(sAhi_s + ks * 256), alo = umma_desc(sAlo_s + ks * 256);
-                    const uint64_t bhi = umma_desc(sBhi_s + ks * 256), blo = umma_desc(sBlo_s + ks * 256);
-                    const uint32_t acc0 = (kc > 0 || ks > 0) ? 1u : 0u;
-                    asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}"
-                                 :: "r"(tmem), "l"(alo), "l"(bhi), "r"(idesc), "r"(acc0) : "memory");
-                    asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}"
-                                 :: "r"(tmem), "l"(ahi), "l"(blo), "r"(idesc), "r"(1u) : "memory");
-                    asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}"
-                                 :: "r"(tmem), "l"(ahi), "l"(bhi), "r"(idesc), "r"(1u) : "memory");
-                }
-                // arrives on the mbarrier when every MMA issued so far has completed (and has finished reading shared memory)
-                asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(mbar_s) : "memory");
-            }
-            {
-                asm volatile("{\n.reg .pred p;\nLAB_WAIT:\nmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra DONE;\nbra LAB_WAIT;\nDONE:\n}"
-                             :: "r"(mbar_s), "r"(phase) : "memory");
-                phase ^= 1u;
-            }
-            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        }
-        // epilogue: warp w reads TMEM lanes 32 w .. 32 w + 31 (= tile rows), 64 columns in two loads of 32
-        const long long row = m0 + warp * 32 + lane;
-#pragma unroll
-        for (int c0 = 0; c0 < kTileN; c0 += 32) {
+    const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(NT >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
+    const int feat = n_base + (warp & 3) * 32 + lane;                       // this thread's output column of w
+    auto epilogue = [&](long long t, int buf) {
+        const long long e0 = t * NT;
+#pragma unroll 1
+        for (int c0 = (warp >> 2) * (NT / 2); c0 < (warp >> 2) * (NT / 2) + NT / 2; c0 += 32) {
             uint32_t v[32];
-            const uint32_t taddr = tmem + ((uint32_t)(warp * 32) << 16) + (uint32_t)c0;
+            const uint32_t taddr = tmem + buf * NT + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)c0;
             asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
                          "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
                          "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
@@ -317,41 +394,192 @@ __global__ void __launch_bounds__(128, 2) radial_gemm_kernel(const float *__rest
                            "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
                          : "r"(taddr) : "memory");
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-            if (row < M) {
-                float *drow = D + row * ldd + n0 + c0;
-                if (n0 + c0 + 32 <= N && (ldd & 3) == 0) {
+            if (feat < N) {
+                float *dp = D + (e0 + c0) * ldd + feat;
+                if (e0 + c0 + 32 <= E) {                 // whole block inside the graph: no per-store predicate
 #pragma unroll
-                    for (int j = 0; j < 32; j += 4)
-                        *reinterpret_cast<float4 *>(drow + j) = make_float4(__uint_as_float(v[j]), __uint_as_float(v[j + 1]), __uint_as_float(v[j + 2]), __uint_as_float(v[j + 3]));
+                    for (int j = 0; j < 32; ++j) { *dp = __uint_as_float(v[j]); dp += ldd; }
                 } else {
 #pragma unroll
                     for (int j = 0; j < 32; ++j)
-                        if (n0 + c0 + j < N) drow[j] = __uint_as_float(v[j]);
+                        if (e0 + c0 + j < E) dp[j * ldd] = __uint_as_float(v[j]);
                 }
             }
         }
-        // the next tile overwrites TMEM and the B tiles: every warp must have drained its TMEM loads first
+    };
+    uint32_t ph0 = 0, ph1 = 0;
+    for (long long t = t_begin; t < t_end; ++t) {
+        const int i = (int)(t - t_begin), buf = i & 1;
+        asm volatile("cp.async.wait_group 0;" ::: "memory");                 // tile t (and, the first time, the slab) has landed
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncthreads();
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        if (tid == 0) {
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            issue_chunk(tmem + buf * NT, sAhi_s, sAlo_s, sB_s + buf * 65536, sB_s + buf * 65536 + 32768, idesc, true, nprod);
+            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(mbar_s + buf * 8) : "memory");
+        }
+        if (i > 0) {                                     // tile t - 1: its MMAs are done -> its operand buffer is free, its accumulators ready
+            const int pb = buf ^ 1;
+            mbar_wait_parity(mbar_s + pb * 8, pb ? ph1 : ph0);
+            if (pb) ph1 ^= 1u; else ph0 ^= 1u;
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        }
+        if (t + 1 < t_end) issue_b(t + 1, buf ^ 1);      // in flight while tile t - 1 drains and the tensor core works on tile t
+        if (i > 0) epilogue(t - 1, buf ^ 1);
     }
+    {
+        const int pb = (int)((t_end - 1 - t_begin) & 1);
+        mbar_wait_parity(mbar_s + pb * 8, pb ? ph1 : ph0);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        epilogue(t_end - 1, pb);
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 256;" :: "r"(tmem) : "memory");
+}
+
+// BACKWARD: D[128-row tile, 64] = sum over K chunks of 64 of A[128 x Kt] * B[64 x Kt]^T (A = grad_weights, fp32, streamed from HBM;
+// B = W3 as TF32 high / low parts).  The chunks are double-buffered in shared memory and the next chunk's loads are in flight in
+// registers while the tensor core works; the accumulator stays in TMEM (64 columns) until the last chunk.
+__global__ void __launch_bounds__(256, 1) radial_gemm_bwd_kernel(const float *__restrict__ A, long long lda, const float *__restrict__ Bhi,
+                                                                 const float *__restrict__ Blo, long long ldb, float *__restrict__ D, long long M, long long Kt)
+{
+    extern __shared__ __align__(1024) unsigned char smem[];                 // 2 stages x (A hi 32 KB, A lo 32 KB, B hi 16 KB, B lo 16 KB)
+    __shared__ __align__(8) unsigned long long mbar[2];
+    __shared__ uint32_t tmem_base_s;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const long long m0 = (long long)blockIdx.x * kTileM;
+    const uint32_t mbar_s = (uint32_t)__cvta_generic_to_shared(&mbar[0]);
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 64;" :: "r"((uint32_t)__cvta_generic_to_shared(&tmem_base_s)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    if (tid == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(mbar_s) : "memory");
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(mbar_s + 8) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem = tmem_base_s;
+    const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(kH >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
+    const uint32_t smem_s = (uint32_t)__cvta_generic_to_shared(smem);
+    const int k_chunks = (int)((Kt + kTileK - 1) / kTileK);
+    // two register stages (chunks kc and kc + 1 are in flight while chunk kc - 1 ... is multiplied): the loads of chunk kc + 2 are issued
+    // right after chunk kc has been written to shared memory and are consumed two iterations later, which hides the DRAM latency
+    float4 ra0[8], rbh0[4], rbl0[4], ra1[8], rbh1[4], rbl1[4];
+    auto load_chunk = [&](int kc, float4 (&ra)[8], float4 (&rbh)[4], float4 (&rbl)[4]) {
+        const long long k0 = (long long)kc * kTileK;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const int row = TILE_ROW(j), q = TILE_QUAD();
+            ra[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (m0 + row < M && k0 + q * 4 + 4 <= Kt) ra[j] = __ldcs(reinterpret_cast<const float4 *>(A + (m0 + row) * lda + k0 + q * 4));
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int row = TILE_ROW(j), q = TILE_QUAD();
+            rbh[j] = make_float4(0.f, 0.f, 0.f, 0.f); rbl[j] = rbh[j];
+            if (k0 + q * 4 + 4 <= Kt) {
+                rbh[j] = __ldg(reinterpret_cast<const float4 *>(Bhi + (long long)row * ldb + k0 + q * 4));
+                rbl[j] = __ldg(reinterpret_cast<const float4 *>(Blo + (long long)row * ldb + k0 + q * 4));
+            }
+        }
+    };
+    auto store_chunk = [&](int buf, const float4 (&ra)[8], const float4 (&rbh)[4], const float4 (&rbl)[4]) {
+        unsigned char *base = smem + buf * 98304;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const int row = TILE_ROW(j), q = TILE_QUAD();
+            const float4 v = ra[j];
+            const float4 h = make_float4(tf32_hi(v.x), tf32_hi(v.y), tf32_hi(v.z), tf32_hi(v.w));
+            const uint32_t off = canon_off(row, q * 4);
+            *reinterpret_cast<float4 *>(base + off) = h;
+            *reinterpret_cast<float4 *>(base + 32768 + off) = make_float4(v.x - h.x, v.y - h.y, v.z - h.z, v.w - h.w);
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int row = TILE_ROW(j), q = TILE_QUAD();
+            const uint32_t off = canon_off(row, q * 4);
+            *reinterpret_cast<float4 *>(base + 65536 + off) = rbh[j];
+            *reinterpret_cast<float4 *>(base + 81920 + off) = rbl[j];
+        }
+    };
+    uint32_t ph0 = 0, ph1 = 0;
+    auto step = [&](int kc, int buf, float4 (&ra)[8], float4 (&rbh)[4], float4 (&rbl)[4], uint32_t &ph) {
+        if (kc >= 2) {                                   // the MMAs of chunk kc - 2 must have finished reading this stage
+            mbar_wait_parity(mbar_s + buf * 8, ph);
+            ph ^= 1u;
+        }
+        store_chunk(buf, ra, rbh, rbl);
+        if (kc + 2 < k_chunks) load_chunk(kc + 2, ra, rbh, rbl);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        if (tid == 0) {
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            const uint32_t b = smem_s + buf * 98304;
+            issue_chunk(tmem, b, b + 32768, b + 65536, b + 81920, idesc, kc == 0);
+            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(mbar_s + buf * 8) : "memory");
+        }
+    };
+    load_chunk(0, ra0, rbh0, rbl0);
+    if (k_chunks > 1) load_chunk(1, ra1, rbh1, rbl1);
+    for (int kc = 0; kc < k_chunks; kc += 2) {
+        step(kc, 0, ra0, rbh0, rbl0, ph0);
+        if (kc + 1 < k_chunks) step(kc + 1, 1, ra1, rbh1, rbl1, ph1);
+    }
+    {   // the last commit covers every MMA issued before it
+        const int buf = (k_chunks - 1) & 1;
+        mbar_wait_parity(mbar_s + buf * 8, buf ? ph1 : ph0);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        epilogue_tile<kH>(tmem, warp, lane, reinterpret_cast<float *>(smem + ((k_chunks & 1) ? 98304 : 0)), D, kH, m0, M, 0, kH);
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 64;" :: "r"(tmem) : "memory");
 }
 
-constexpr int kGemmSmem = 65536 + 32768;
+constexpr int kGemmSmem = 196608;      // forward: A 64 KB + 2 x 64 KB of B; backward: 2 x 96 KB stages (the epilogue stages through an idle buffer)
 
-int launch_gemm(const float *A, long long lda, const float *Bhi, const float *Blo, long long ldb, float *D, long long ldd, long long M, int N,
-                int n_tiles, int k_chunks, long long Kt, cudaStream_t st)
+int launch_gemm_fwd(const float *Hhi, const float *Hlo, const float *W3Thi, const float *W3Tlo, float *D, long long ldd, long long E, int N, cudaStream_t st)
 {
     static bool attr_set = false;
     if (!attr_set) {
-        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
+        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
+        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
+        attr_set = true;
+    }
+    if (E <= 0) return E3_OK;
+    // grid: (feature slabs of 128) x (runs of edge tiles): a CTA keeps its slab for `tiles_per_cta` 128-edge tiles; enough CTAs for
+    // ~8 per SM so that the slabs of one edge range run together (the h2 rows they share stay in L2)
+    const int slabs = (N + kTileM - 1) / kTileM;
+    const long long n_etiles = (E + 127) / 128;
+    long long runs = (148LL * 8 + slabs - 1) / slabs;
+    if (runs > n_etiles) runs = n_etiles;
+    const int tiles_per_cta = (int)((n_etiles + runs - 1) / runs);
+    runs = (n_etiles + tiles_per_cta - 1) / tiles_per_cta;
+    if (runs > 65535) { set_error("radial gemm: grid too large"); return E3_ERR_UNSUPPORTED; }
+    static const int nprod = []() { const char *e = getenv("E3_RADIAL_PRODUCTS"); return (e && e[0] == '1') ? 1 : 3; }();
+    radial_gemm_fwd_kernel<<<dim3((unsigned)slabs, (unsigned)runs), 256, kGemmSmem, st>>>(Hhi, Hlo, W3Thi, W3Tlo, D, ldd, E, N, tiles_per_cta, nprod);
+    E3_CUDA_TRY(cudaGetLastError());
+    return E3_OK;
+}
+
+int launch_gemm_bwd(const float *A, long long lda, const float *Bhi, const float *Blo, long long ldb, float *D, long long M, long long Kt, cudaStream_t st)
+{
+    static bool attr_set = false;
+    if (!attr_set) {
+        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
+        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
         attr_set = true;
     }
     if (M <= 0) return E3_OK;
     const long long grid = (M + kTileM - 1) / kTileM;
     if (grid > 0x7fffffffLL) { set_error("radial gemm: grid too large"); return E3_ERR_UNSUPPORTED; }
-    radial_gemm_kernel<<<(unsigned)grid, 128, kGemmSmem, st>>>(A, lda, Bhi, Blo, ldb, D, ldd, M, N, n_tiles, k_chunks, Kt);
+    radial_gemm_bwd_kernel<<<(unsigned)grid, 256, kGemmSmem, st>>>(A, lda, Bhi, Blo, ldb, D, M, Kt);
     E3_CUDA_TRY(cudaGetLastError());
     return E3_OK;
 }
@@ -414,7 +642,7 @@ extern "C" int e3_radial_create(e3_radial **net, int num_rbf, int envelope_p, do
 extern "C" size_t e3_radial_workspace_bytes(const e3_radial *net, int64_t n_edges)
 {
     if (!net || n_edges < 0) return 0;
-    return (size_t)n_edges * kH * sizeof(float) + 256;       // h2 (forward) or dh2 (backward), [E,64] fp32
+    return (size_t)n_edges * kH * sizeof(float) * 2 + 256;   // h2 as TF32 high / low parts (forward), dh2 (backward): [E,64] fp32 each
 }
 
 extern "C" int e3_radial_weights_fwd(const e3_radial *net, const float *vec, int64_t n_edges, float *weights, void *workspace,
@@ -426,10 +654,11 @@ extern "C" int e3_radial_weights_fwd(const e3_radial *net, const float *vec, int
     if ((reinterpret_cast<uintptr_t>(weights) & 15u) || (reinterpret_cast<uintptr_t>(workspace) & 15u)) { set_error("e3_radial_weights_fwd: pointers must be 16-byte aligned"); return E3_ERR_INVALID_ARG; }
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     float *h2 = reinterpret_cast<float *>(workspace);
-    const long long blocks = std::min<long long>((n_edges + 3) / 4, 148LL * 16);
-    radial_hidden_kernel<<<(unsigned)blocks, 128, 0, st>>>(vec, n_edges, net->K, net->p, (float)net->rc, net->W1, net->W2, h2);
+    const long long blocks = std::min<long long>((n_edges + 15) / 16, 148LL * 8);
+    radial_hidden_kernel<false><<<(unsigned)blocks, 128, kHiddenSmemFwd, st>>>(vec, n_edges, net->K, net->p, (float)net->rc, net->W1, net->W2, net->W2T, h2,
+                                                                                nullptr, nullptr, 0);
     E3_CUDA_TRY(cudaGetLastError());
-    return launch_gemm(h2, kH, net->W3T_hi, net->W3T_lo, kH, weights, net->n_out, n_edges, net->n_out, (net->n_out + kTileN - 1) / kTileN, 1, kH, st);
+    return launch_gemm_fwd(h2, h2 + (size_t)n_edges * kH, net->W3T_hi, net->W3T_lo, weights, net->n_out, n_edges, net->n_out, st);
 }
 
 extern "C" int e3_radial_weights_bwd(const e3_radial *net, const float *vec, int64_t n_edges, const float *grad_weights, float *grad_vec,
@@ -442,10 +671,11 @@ extern "C" int e3_radial_weights_bwd(const e3_radial *net, const float *vec, int
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     float *dh2 = reinterpret_cast<float *>(workspace);
     // dh2[E,64] = dw[E,n_out] * W3[64,n_out]^T : A = dw (K = n_out), B = W3 rows (K-major), one N tile, n_out / 64 K chunks
-    int rc = launch_gemm(grad_weights, net->n_out, net->W3_hi, net->W3_lo, net->n_out, dh2, kH, n_edges, kH, 1, (net->n_out + kTileK - 1) / kTileK, net->n_out, st);
+    int rc = launch_gemm_bwd(grad_weights, net->n_out, net->W3_hi, net->W3_lo, net->n_out, dh2, n_edges, net->n_out, st);
     if (rc != E3_OK) return rc;
-    const long long blocks = std::min<long long>((n_edges + 3) / 4, 148LL * 16);
-    radial_hidden_bwd_kernel<<<(unsigned)blocks, 128, 0, st>>>(vec, n_edges, net->K, net->p, (float)net->rc, net->W1, net->W2, net->W2T, dh2, grad_vec, accumulate);
+    const long long blocks = std::min<long long>((n_edges + 15) / 16, 148LL * 8);
+    radial_hidden_kernel<true><<<(unsigned)blocks, 128, kHiddenSmemBwd, st>>>(vec, n_edges, net->K, net->p, (float)net->rc, net->W1, net->W2, net->W2T, nullptr,
+                                                                               dh2, grad_vec, accumulate);
     E3_CUDA_TRY(cudaGetLastError());
     return E3_OK;
 }
