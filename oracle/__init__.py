@@ -258,3 +258,70 @@ def radial_weights_bwd(vec, K, p, rc, W1, W2, W3, dw):
     dr = (df * dfdr).sum(1)
     rhat = np.where(r[:, None] > 0, vec / np.where(r > 0, r, 1.0)[:, None], 0.0)
     return dr[:, None] * rhat, dW1, dW2, dW3
+
+
+# --------------------------------------------------------------------------------------------
+# NEXT-4 / NEXT-2: per-irrep multiplicities, second-order VJP, SH second derivative (e3_oracle_next.c)
+# --------------------------------------------------------------------------------------------
+def tp_mul_dims(irreps_in, sh_lmax, irreps_out, paths):
+    a = _plan_args(irreps_in, sh_lmax, irreps_out, paths)
+    v = [C.c_int() for _ in range(4)]
+    rc = _L().orc_tp_mul_dims(*a, *[C.byref(t) for t in v])
+    if rc:
+        raise ValueError(f"oracle plan invalid (code {rc})")
+    return tuple(t.value for t in v)          # in_size, sh_dim, out_size, w_size (elements per row)
+
+
+def tp_mul_fwd(irreps_in, sh_lmax, irreps_out, paths, x, Y, w, senders, receivers, n_nodes):
+    """Forward with per-irrep multiplicities (NEXT-4); rows are in_size / out_size / w_size elements wide."""
+    a = _plan_args(irreps_in, sh_lmax, irreps_out, paths)
+    in_size, sh_dim, out_size, w_size = tp_mul_dims(irreps_in, sh_lmax, irreps_out, paths)
+    x, Y, w = _f64(x), _f64(Y), _f64(w)
+    senders, receivers = _i32(senders), _i32(receivers)
+    E = senders.shape[0]
+    assert x.size == n_nodes * in_size and Y.size == E * sh_dim and w.size == E * w_size
+    out = np.empty((n_nodes, out_size))
+    rc = _L().orc_tp_mul_fwd(*a, _p(x), _p(Y), _p(w), _p(senders), _p(receivers), C.c_int64(E), C.c_int32(n_nodes), _p(out))
+    if rc:
+        raise ValueError(f"oracle plan invalid (code {rc})")
+    return out
+
+
+def tp_mul_bwd(irreps_in, sh_lmax, irreps_out, paths, x, Y, w, senders, receivers, n_nodes, g):
+    a = _plan_args(irreps_in, sh_lmax, irreps_out, paths)
+    in_size, sh_dim, out_size, w_size = tp_mul_dims(irreps_in, sh_lmax, irreps_out, paths)
+    x, Y, w, g = _f64(x), _f64(Y), _f64(w), _f64(g)
+    senders, receivers = _i32(senders), _i32(receivers)
+    E = senders.shape[0]
+    dx, dY, dw = np.empty((n_nodes, in_size)), np.empty((E, sh_dim)), np.empty((E, w_size))
+    rc = _L().orc_tp_mul_bwd(*a, _p(x), _p(Y), _p(w), _p(senders), _p(receivers), C.c_int64(E), C.c_int32(n_nodes), _p(g),
+                             _p(dx), _p(dY), _p(dw))
+    if rc:
+        raise ValueError(f"oracle plan invalid (code {rc})")
+    return dx, dY, dw
+
+
+def tp_vjp_vjp(irreps_in, sh_lmax, irreps_out, paths, x, Y, w, senders, receivers, n_nodes, g, vx, vY, vw):
+    """(gg, gx, gY, gw): gradients of S = <vx,dx> + <vY,dY> + <vw,dw> (NEXT-2, section 5.2)."""
+    a = _plan_args(irreps_in, sh_lmax, irreps_out, paths)
+    in_size, sh_dim, out_size, w_size = tp_mul_dims(irreps_in, sh_lmax, irreps_out, paths)
+    x, Y, w, g, vx, vY, vw = (_f64(t) for t in (x, Y, w, g, vx, vY, vw))
+    senders, receivers = _i32(senders), _i32(receivers)
+    E = senders.shape[0]
+    gg, gx, gY, gw = np.empty((n_nodes, out_size)), np.empty((n_nodes, in_size)), np.empty((E, sh_dim)), np.empty((E, w_size))
+    rc = _L().orc_tp_vjp_vjp(*a, _p(x), _p(Y), _p(w), _p(senders), _p(receivers), C.c_int64(E), C.c_int32(n_nodes), _p(g),
+                             _p(vx), _p(vY), _p(vw), _p(gg), _p(gx), _p(gY), _p(gw))
+    if rc:
+        raise ValueError(f"oracle plan invalid (code {rc})")
+    return gg, gx, gY, gw
+
+
+def sh_bwd_bwd(lmax, vec, dY, u):
+    """VJP of (vec, dY) -> J(vec)^T dY for a cotangent u[n,3]: (g_vec[n,3], g_dY[n,(lmax+1)^2])."""
+    vec, dY, u = _f64(vec).reshape(-1, 3), _f64(dY), _f64(u).reshape(-1, 3)
+    n = vec.shape[0]
+    gv, gd = np.empty((n, 3)), np.empty((n, (lmax + 1) ** 2))
+    rc = _L().orc_sh_bwd_bwd(C.c_int(lmax), C.c_int64(n), _p(vec), _p(dY), _p(u), _p(gv), _p(gd))
+    if rc:
+        raise ValueError("lmax out of range")
+    return gv, gd

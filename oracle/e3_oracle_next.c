@@ -134,3 +134,258 @@ void orc_radial_mlp_bwd(int K, int H, int M, int64_t n, const double *f, const d
     }
     free(a1); free(h1); free(a2); free(h2); free(g2); free(g1);
 }
+
+/* =================================================================================================================
+ * General-multiplicity plan used by the NEXT-2 / NEXT-4 functions below.  Reading A7 generalised (NEXT-4, PAPER.md L484-L485:
+ * NequIP `target_irreps 64x0e + 64x0o + 32x1o + 32x1e + 32x2e + 32x2o`): every irrep i has its own multiplicity mul_i; a node row is
+ * the concatenation of blocks of (2l_i+1)*mul_i elements, index m*mul_i + u inside a block; a path ("uvu") needs
+ * mul(i_in) == mul(i_out) and owns mul weights per edge, stored path after path: w[e, w_off(p) + u].
+ * ================================================================================================================= */
+typedef struct { int l; int parity; int mul; } nx_irrep;
+typedef struct { int i_in; int l_sh; int i_out; } nx_path;
+double orc_cg_real(int l1, int l2, int l3, double *C);      /* e3_oracle.c (reading A4) */
+
+typedef struct {
+    int n_paths, in_size, out_size, sh_dim, w_size;
+    int l1[256], l2[256], l3[256], mul[256], in_off[256], out_off[256], w_off[256];
+    double *cg[256];
+} nplan;
+
+static void nplan_free(nplan *pl) { for (int p = 0; p < pl->n_paths; ++p) free(pl->cg[p]); }
+
+static int nplan_build(nplan *pl, const nx_irrep *ii, int n_in, int sh_lmax, const nx_irrep *io, int n_out, const nx_path *paths, int n_paths)
+{
+    int in_off[256], out_off[256];
+    pl->n_paths = 0;
+    if (n_paths > 256 || n_in > 256 || n_out > 256 || n_in < 1 || n_out < 1) return 1;
+    pl->in_size = 0;
+    for (int i = 0; i < n_in; ++i) { in_off[i] = pl->in_size; pl->in_size += (2 * ii[i].l + 1) * ii[i].mul; }
+    pl->out_size = 0;
+    for (int i = 0; i < n_out; ++i) { out_off[i] = pl->out_size; pl->out_size += (2 * io[i].l + 1) * io[i].mul; }
+    pl->sh_dim = (sh_lmax + 1) * (sh_lmax + 1);
+    pl->w_size = 0;
+    for (int p = 0; p < n_paths; ++p) pl->cg[p] = NULL;
+    pl->n_paths = n_paths;
+    for (int p = 0; p < n_paths; ++p) {
+        nx_path q = paths[p];
+        if (q.i_in < 0 || q.i_in >= n_in || q.i_out < 0 || q.i_out >= n_out || q.l_sh < 0 || q.l_sh > sh_lmax) return 3;
+        const int l1 = ii[q.i_in].l, l2 = q.l_sh, l3 = io[q.i_out].l;
+        if (l3 < abs(l1 - l2) || l3 > l1 + l2) return 4;
+        if (ii[q.i_in].parity * ((l2 & 1) ? -1 : 1) != io[q.i_out].parity) return 5;
+        if (ii[q.i_in].mul != io[q.i_out].mul || ii[q.i_in].mul < 1) return 2;
+        pl->l1[p] = l1; pl->l2[p] = l2; pl->l3[p] = l3; pl->mul[p] = ii[q.i_in].mul;
+        pl->in_off[p] = in_off[q.i_in]; pl->out_off[p] = out_off[q.i_out];
+        pl->w_off[p] = pl->w_size; pl->w_size += pl->mul[p];
+        pl->cg[p] = (double *)malloc(sizeof(double) * (size_t)((2 * l1 + 1) * (2 * l2 + 1) * (2 * l3 + 1)));
+        orc_cg_real(l1, l2, l3, pl->cg[p]);
+    }
+    return 0;
+}
+
+int orc_tp_mul_dims(const nx_irrep *ii, int n_in, int sh_lmax, const nx_irrep *io, int n_out, const nx_path *paths, int n_paths,
+                    int *in_size, int *sh_dim, int *out_size, int *w_size)
+{
+    nplan pl;
+    int rc = nplan_build(&pl, ii, n_in, sh_lmax, io, n_out, paths, n_paths);
+    if (!rc) { *in_size = pl.in_size; *sh_dim = pl.sh_dim; *out_size = pl.out_size; *w_size = pl.w_size; }
+    nplan_free(&pl);
+    return rc;
+}
+
+/* NEXT-4: forward with per-irrep multiplicities (the definition of SURVEY 8(c) with C replaced by mul(p)):
+ *   out[r, out_off(p) + m3*mul + u] += w[e, w_off(p)+u] * C^p[m1,m2,m3] * x[snd(e), in_off(p) + m1*mul + u] * Y[e, l2^2 + m2]
+ * Pins (tests/test_oracle_next.py): equals orc_tp_scatter_fwd for equal multiplicities; brute-force einsum; a plan whose irreps
+ * fall into multiplicity classes equals the independent equal-multiplicity plans of the classes. */
+int orc_tp_mul_fwd(const nx_irrep *ii, int n_in, int sh_lmax, const nx_irrep *io, int n_out, const nx_path *paths, int n_paths,
+                   const double *x, const double *sh, const double *w, const int32_t *senders, const int32_t *receivers, int64_t E, int32_t N, double *out)
+{
+    nplan pl;
+    int rc = nplan_build(&pl, ii, n_in, sh_lmax, io, n_out, paths, n_paths);
+    if (rc) { nplan_free(&pl); return rc; }
+    memset(out, 0, sizeof(double) * (size_t)N * pl.out_size);
+    for (int64_t e = 0; e < E; ++e) {
+        const double *xs = x + (int64_t)senders[e] * pl.in_size, *Ye = sh + e * pl.sh_dim, *we = w + e * pl.w_size;
+        double *o = out + (int64_t)receivers[e] * pl.out_size;
+        for (int p = 0; p < pl.n_paths; ++p) {
+            const int l1 = pl.l1[p], l2 = pl.l2[p], l3 = pl.l3[p], mu = pl.mul[p], d2 = 2 * l2 + 1, d3 = 2 * l3 + 1;
+            for (int m1 = 0; m1 <= 2 * l1; ++m1)
+                for (int m2 = 0; m2 <= 2 * l2; ++m2)
+                    for (int m3 = 0; m3 <= 2 * l3; ++m3) {
+                        const double c = pl.cg[p][(m1 * d2 + m2) * d3 + m3];
+                        if (c == 0.0) continue;
+                        for (int u = 0; u < mu; ++u)
+                            o[pl.out_off[p] + m3 * mu + u] += we[pl.w_off[p] + u] * c * xs[pl.in_off[p] + m1 * mu + u] * Ye[l2 * l2 + m2];
+                    }
+        }
+    }
+    nplan_free(&pl);
+    return 0;
+}
+
+/* NEXT-4: the three VJP contractions of SURVEY 8(a) a5 with per-irrep multiplicities. */
+int orc_tp_mul_bwd(const nx_irrep *ii, int n_in, int sh_lmax, const nx_irrep *io, int n_out, const nx_path *paths, int n_paths,
+                   const double *x, const double *sh, const double *w, const int32_t *senders, const int32_t *receivers, int64_t E, int32_t N,
+                   const double *g, double *dx, double *dY, double *dw)
+{
+    nplan pl;
+    int rc = nplan_build(&pl, ii, n_in, sh_lmax, io, n_out, paths, n_paths);
+    if (rc) { nplan_free(&pl); return rc; }
+    memset(dx, 0, sizeof(double) * (size_t)N * pl.in_size);
+    memset(dY, 0, sizeof(double) * (size_t)E * pl.sh_dim);
+    memset(dw, 0, sizeof(double) * (size_t)E * pl.w_size);
+    for (int64_t e = 0; e < E; ++e) {
+        const int64_t s = senders[e], r = receivers[e];
+        for (int p = 0; p < pl.n_paths; ++p) {
+            const int l1 = pl.l1[p], l2 = pl.l2[p], l3 = pl.l3[p], mu = pl.mul[p], d2 = 2 * l2 + 1, d3 = 2 * l3 + 1;
+            for (int m1 = 0; m1 <= 2 * l1; ++m1)
+                for (int m2 = 0; m2 <= 2 * l2; ++m2)
+                    for (int m3 = 0; m3 <= 2 * l3; ++m3) {
+                        const double c = pl.cg[p][(m1 * d2 + m2) * d3 + m3];
+                        if (c == 0.0) continue;
+                        for (int u = 0; u < mu; ++u) {
+                            const double xv = x[s * pl.in_size + pl.in_off[p] + m1 * mu + u], Yv = sh[e * pl.sh_dim + l2 * l2 + m2];
+                            const double wv = w[e * pl.w_size + pl.w_off[p] + u], gv = g[r * pl.out_size + pl.out_off[p] + m3 * mu + u];
+                            dx[s * pl.in_size + pl.in_off[p] + m1 * mu + u] += c * Yv * wv * gv;
+                            dY[e * pl.sh_dim + l2 * l2 + m2] += c * xv * wv * gv;
+                            dw[e * pl.w_size + pl.w_off[p] + u] += c * xv * Yv * gv;
+                        }
+                    }
+        }
+    }
+    nplan_free(&pl);
+    return 0;
+}
+
+/* NEXT-2: VJP of the VJP (section 5.2, Eq. 3-4: a Hessian row is a reverse-mode derivative of selected force
+ * components, i.e. of first-order VJP outputs).  The forward is trilinear, T = sum C x Y w, and the first-order outputs for a cotangent g
+ * are dx = sum C Y w g, dY = sum C x w g, dw = sum C x Y g.  For cotangents (vx, vY, vw) of (dx, dY, dw) the scalar
+ *   S = <vx, dx> + <vY, dY> + <vw, dw> = sum C g (vx Y w + x vY w + x Y vw)
+ * has the gradients written out below (each is S with one factor removed):
+ *   gg = dS/dg, gx = dS/dx, gY = dS/dY, gw = dS/dw.
+ * Pins: central differences of S built from the (pinned) first-order oracle in every input; gg = T(vx,Y,w) + T(x,vY,w) + T(x,Y,vw)
+ * through orc_tp_scatter_fwd; symmetry of the second derivative. */
+int orc_tp_vjp_vjp(const nx_irrep *ii, int n_in, int sh_lmax, const nx_irrep *io, int n_out, const nx_path *paths, int n_paths,
+                   const double *x, const double *sh, const double *w, const int32_t *senders, const int32_t *receivers, int64_t E, int32_t N,
+                   const double *g, const double *vx, const double *vY, const double *vw,
+                   double *gg, double *gx, double *gY, double *gw)
+{
+    nplan pl;
+    int rc = nplan_build(&pl, ii, n_in, sh_lmax, io, n_out, paths, n_paths);
+    if (rc) { nplan_free(&pl); return rc; }
+    memset(gg, 0, sizeof(double) * (size_t)N * pl.out_size);
+    memset(gx, 0, sizeof(double) * (size_t)N * pl.in_size);
+    memset(gY, 0, sizeof(double) * (size_t)E * pl.sh_dim);
+    memset(gw, 0, sizeof(double) * (size_t)E * pl.w_size);
+    for (int64_t e = 0; e < E; ++e) {
+        const int64_t s = senders[e], r = receivers[e];
+        for (int p = 0; p < pl.n_paths; ++p) {
+            const int l1 = pl.l1[p], l2 = pl.l2[p], l3 = pl.l3[p], mu = pl.mul[p], d2 = 2 * l2 + 1, d3 = 2 * l3 + 1;
+            for (int m1 = 0; m1 <= 2 * l1; ++m1)
+                for (int m2 = 0; m2 <= 2 * l2; ++m2)
+                    for (int m3 = 0; m3 <= 2 * l3; ++m3) {
+                        const double c = pl.cg[p][(m1 * d2 + m2) * d3 + m3];
+                        if (c == 0.0) continue;
+                        for (int u = 0; u < mu; ++u) {
+                            const int64_t ix = s * pl.in_size + pl.in_off[p] + m1 * mu + u, iy = e * pl.sh_dim + l2 * l2 + m2;
+                            const int64_t iw = e * pl.w_size + pl.w_off[p] + u, ig = r * pl.out_size + pl.out_off[p] + m3 * mu + u;
+                            const double xv = x[ix], Yv = sh[iy], wv = w[iw], gv = g[ig], a = vx[ix], b = vY[iy], d = vw[iw];
+                            gg[ig] += c * (a * Yv * wv + xv * b * wv + xv * Yv * d);
+                            gx[ix] += c * gv * (b * wv + Yv * d);
+                            gY[iy] += c * gv * (a * wv + xv * d);
+                            gw[iw] += c * gv * (a * Yv + xv * b);
+                        }
+                    }
+        }
+    }
+    nplan_free(&pl);
+    return 0;
+}
+
+/* NEXT-2: second derivative of the spherical harmonics, as the VJP of  (vec, dY) -> dvec = J(vec)^T dY  (orc_sh_bwd) for a
+ * cotangent u[n,3]:   g_dY[n,lm] = J(vec) u   and   g_vec = (sum_lm dY_lm Hess Y_lm(vec)) u.
+ * Y_lm(vec) = P_lm(vec) / |vec|^l with the homogeneous polynomials P_lm of reading A2 (the explicit forms with 1 written as r^2), kept
+ * here as monomial tables; gradient and Hessian follow from
+ *   grad f = grad P r^-l - l P r^-(l+2) v,
+ *   Hess f = Hess P r^-l - l (grad P v^T + v grad P^T) r^-(l+2) - l P r^-(l+2) I + l (l+2) P r^-(l+4) v v^T.
+ * A zero vector gives zeros (reading A3).  Pins: P/r^l equals orc_sh; g_dY equals orc_sh_jac applied to u; g_vec equals central
+ * differences of orc_sh_bwd; Hess is symmetric and annihilates ... r (degree-0 homogeneity: Hess f v = -grad f). */
+typedef struct { double c; int a, b, d; } mono;   /* c x^a y^b z^d */
+#define S3 1.7320508075688772935
+#define S5 2.2360679774997896964
+#define S7 2.6457513110645905905
+#define S15 3.8729833462074168852
+#define S42 6.4807406984078602310
+#define S70 8.3666002653407554798
+#define S105 10.246950765959598383
+static const mono P00[] = { { 1.0, 0, 0, 0 } };
+static const mono P1m[] = { { S3, 0, 1, 0 } }, P10[] = { { S3, 0, 0, 1 } }, P1p[] = { { S3, 1, 0, 0 } };
+static const mono P2a[] = { { S15, 1, 1, 0 } }, P2b[] = { { S15, 0, 1, 1 } };
+static const mono P2c[] = { { S5, 0, 0, 2 }, { -0.5 * S5, 2, 0, 0 }, { -0.5 * S5, 0, 2, 0 } };          /* (sqrt5/2)(3z^2 - r^2) */
+static const mono P2d[] = { { S15, 1, 0, 1 } }, P2e[] = { { 0.5 * S15, 2, 0, 0 }, { -0.5 * S15, 0, 2, 0 } };
+static const mono P3a[] = { { 0.75 * S70, 2, 1, 0 }, { -0.25 * S70, 0, 3, 0 } };                          /* (sqrt70/4) y (3x^2 - y^2) */
+static const mono P3b[] = { { S105, 1, 1, 1 } };
+static const mono P3c[] = { { S42, 0, 1, 2 }, { -0.25 * S42, 2, 1, 0 }, { -0.25 * S42, 0, 3, 0 } };      /* (sqrt42/4) y (5z^2 - r^2) */
+static const mono P3d[] = { { S7, 0, 0, 3 }, { -1.5 * S7, 2, 0, 1 }, { -1.5 * S7, 0, 2, 1 } };           /* (sqrt7/2) z (5z^2 - 3r^2) */
+static const mono P3e[] = { { S42, 1, 0, 2 }, { -0.25 * S42, 3, 0, 0 }, { -0.25 * S42, 1, 2, 0 } };      /* (sqrt42/4) x (5z^2 - r^2) */
+static const mono P3f[] = { { 0.5 * S105, 2, 0, 1 }, { -0.5 * S105, 0, 2, 1 } };
+static const mono P3g[] = { { 0.25 * S70, 3, 0, 0 }, { -0.75 * S70, 1, 2, 0 } };                          /* (sqrt70/4) x (x^2 - 3y^2) */
+static const mono *const PT[16] = { P00, P1m, P10, P1p, P2a, P2b, P2c, P2d, P2e, P3a, P3b, P3c, P3d, P3e, P3f, P3g };
+static const int PN[16] = { 1, 1, 1, 1, 1, 1, 3, 1, 2, 2, 1, 3, 3, 3, 2, 2 };
+static const int PL[16] = { 0, 1, 1, 1, 2, 2, 2, 2, 2, 3, 3, 3, 3, 3, 3, 3 };
+
+static double ipow(double t, int n) { double r = 1.0; for (int i = 0; i < n; ++i) r *= t; return r; }
+
+/* value, gradient and Hessian of the polynomial P_lm at v */
+static void poly_eval(int lm, const double *v, double *P, double *gP, double *HP)
+{
+    *P = 0.0;
+    for (int i = 0; i < 3; ++i) gP[i] = 0.0;
+    for (int i = 0; i < 9; ++i) HP[i] = 0.0;
+    for (int t = 0; t < PN[lm]; ++t) {
+        const mono m = PT[lm][t];
+        const int ex[3] = { m.a, m.b, m.d };
+        *P += m.c * ipow(v[0], ex[0]) * ipow(v[1], ex[1]) * ipow(v[2], ex[2]);
+        for (int i = 0; i < 3; ++i) {
+            if (ex[i] < 1) continue;
+            int e1[3] = { ex[0], ex[1], ex[2] };
+            e1[i] -= 1;
+            const double ci = m.c * ex[i];
+            gP[i] += ci * ipow(v[0], e1[0]) * ipow(v[1], e1[1]) * ipow(v[2], e1[2]);
+            for (int j = 0; j < 3; ++j) {
+                if (e1[j] < 1) continue;
+                int e2[3] = { e1[0], e1[1], e1[2] };
+                e2[j] -= 1;
+                HP[i * 3 + j] += ci * e1[j] * ipow(v[0], e2[0]) * ipow(v[1], e2[1]) * ipow(v[2], e2[2]);
+            }
+        }
+    }
+}
+
+int orc_sh_bwd_bwd(int lmax, int64_t n, const double *vec, const double *dY, const double *u, double *g_vec, double *g_dY)
+{
+    if (lmax < 0 || lmax > 3) return 1;
+    const int D = (lmax + 1) * (lmax + 1);
+    for (int64_t i = 0; i < n; ++i) {
+        const double *v = vec + 3 * i, *ui = u + 3 * i;
+        double *gv = g_vec + 3 * i;
+        gv[0] = gv[1] = gv[2] = 0.0;
+        const double r2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
+        if (!(r2 > 0.0)) { for (int k = 0; k < D; ++k) g_dY[i * D + k] = 0.0; continue; }
+        const double r = sqrt(r2);
+        for (int lm = 0; lm < D; ++lm) {
+            const int l = PL[lm];
+            double P, gP[3], HP[9];
+            poly_eval(lm, v, &P, gP, HP);
+            const double rl = ipow(r, l);
+            double grad[3], H[9];
+            for (int a = 0; a < 3; ++a) grad[a] = gP[a] / rl - l * P / (rl * r2) * v[a];
+            for (int a = 0; a < 3; ++a)
+                for (int b = 0; b < 3; ++b)
+                    H[a * 3 + b] = HP[a * 3 + b] / rl - l * (gP[a] * v[b] + v[a] * gP[b]) / (rl * r2) - (a == b ? l * P / (rl * r2) : 0.0)
+                                   + l * (l + 2) * P / (rl * r2 * r2) * v[a] * v[b];
+            g_dY[i * D + lm] = grad[0] * ui[0] + grad[1] * ui[1] + grad[2] * ui[2];
+            for (int a = 0; a < 3; ++a) gv[a] += dY[i * D + lm] * (H[a * 3] * ui[0] + H[a * 3 + 1] * ui[1] + H[a * 3 + 2] * ui[2]);
+        }
+    }
+    return 0;
+}
