@@ -232,6 +232,29 @@ int e3_radial_weights_fwd(const e3_radial *net, const float *vec /*[E,3]*/, int6
 int e3_radial_weights_bwd(const e3_radial *net, const float *vec, int64_t n_edges, const float *grad_weights /*[E,n_out]*/,
                           float *grad_vec /*[E,3]*/, int accumulate, void *workspace, size_t workspace_bytes, e3_stream stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * NEXT-2: second-order VJP, for Hessian rows and Hessian-label training.  PAPER.md L108-L126 (section 5.2),
+ * Eq. 3 (H_ij = d2E/dr_i dr_j = -dF_i/dr_j) and Eq. 4 (rows of selected force components by reverse mode): a Hessian row is
+ * the VJP of first-order VJP outputs.  With out = T(feats, sh, weights) (trilinear) and the first-order outputs
+ * (grad_feats, grad_sh, grad_weights) of e3_tp_scatter_bwd for the cotangent grad_out, let
+ *   S = <v_feats, grad_feats> + <v_sh, grad_sh> + <v_weights, grad_weights>.
+ * e3_tp_scatter_vjp_vjp returns dS/d grad_out (gg_out [N,out_dim*C]), dS/d feats (g_feats [N,in_dim*C]), dS/d sh (g_sh
+ * [E,sh_dim]) and dS/d weights (g_weights [E,P*C]), all float.  Any of v_feats / v_sh / v_weights may be NULL (= zero) and any
+ * output may be NULL (not computed).  Built from the plan's forward and VJP kernels with one operand replaced by its cotangent
+ * (exact, because T is trilinear); E3_F32 plans only (E3_ERR_UNSUPPORTED otherwise).  workspace >= e3_vjp_vjp_workspace_bytes.
+ * e3_sh_bwd_bwd is the matching second derivative of the spherical harmonics: the VJP of (vec, grad_sh) -> grad_vec of
+ * e3_sh_bwd for a cotangent u[E,3]:  g_sh[E,sh_dim] = J(vec) u  and  g_vec[E,3] = (sum_lm grad_sh[e,lm] Hess Y_lm(vec_e)) u_e
+ * (zeros for a zero-length vector); either output may be NULL.
+ * -------------------------------------------------------------------------------------------*/
+size_t e3_vjp_vjp_workspace_bytes(const e3_plan *plan, int64_t n_edges, int32_t n_nodes);
+int e3_tp_scatter_vjp_vjp(const e3_plan *plan, const void *feats, const void *sh, const void *weights, const int32_t *senders,
+                          const int32_t *receivers, const int32_t *row_ptr, const int32_t *perm_s, const int32_t *col_ptr,
+                          int64_t n_edges, int32_t n_nodes, const float *grad_out, const float *v_feats, const float *v_sh,
+                          const float *v_weights, float *gg_out, float *g_feats, float *g_sh, float *g_weights,
+                          void *workspace, size_t workspace_bytes, e3_stream stream);
+int e3_sh_bwd_bwd(const e3_plan *plan, const float *vec, const float *grad_sh, const float *u, int64_t n_edges,
+                  float *g_vec, float *g_sh, e3_stream stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -23,6 +23,7 @@ SYMBOLS = [
     "e3_plan_get_cg", "e3_plan_kernel_info", "e3_plan_work", "e3_jit_check", "e3_graph_workspace_bytes",
     "e3_graph_prepare", "e3_sh_fwd", "e3_sh_bwd", "e3_tp_scatter_fwd", "e3_bwd_workspace_bytes", "e3_tp_scatter_bwd",
     "e3_force_reduce", "e3_profile_set_mid_event", "e3_measure_fp32_peak", "e3_session_create", "e3_session_destroy", "e3_session_run_host",
+    "e3_vjp_vjp_workspace_bytes", "e3_tp_scatter_vjp_vjp", "e3_sh_bwd_bwd",
     "e3_radial_create", "e3_radial_destroy", "e3_radial_workspace_bytes", "e3_radial_weights_fwd", "e3_radial_weights_bwd",
 ]
 
@@ -57,6 +58,8 @@ def lib():
         L.e3_graph_workspace_bytes.argtypes = [C.c_int64, C.c_int32]
         L.e3_bwd_workspace_bytes.restype = C.c_size_t
         L.e3_bwd_workspace_bytes.argtypes = [C.c_void_p, C.c_int64, C.c_int32]
+        L.e3_vjp_vjp_workspace_bytes.restype = C.c_size_t
+        L.e3_vjp_vjp_workspace_bytes.argtypes = [C.c_void_p, C.c_int64, C.c_int32]
         L.e3_radial_workspace_bytes.restype = C.c_size_t
         L.e3_radial_workspace_bytes.argtypes = [C.c_void_p, C.c_int64]
         _lib = L
@@ -336,3 +339,31 @@ def e3_radial_weights_bwd(net: Radial, vec, grad_weights, grad_vec=None, accumul
     _check(lib().e3_radial_weights_bwd(net.handle, _ptr(vec), C.c_int64(E), _ptr(grad_weights), _ptr(_dev(gv, torch.float32)),
                                        int(bool(accumulate)), _ptr(ws), C.c_size_t(ws.numel()), _stream(stream)), "e3_radial_weights_bwd")
     return gv
+
+
+def e3_tp_scatter_vjp_vjp(plan: Plan, feats, sh, weights, senders, receivers, row_ptr, perm_s, col_ptr, n_nodes, grad_out,
+                          v_feats=None, v_sh=None, v_weights=None, want=("gg", "gx", "gY", "gw"), stream=None):
+    """Second-order VJP (NEXT-2).  Returns a dict with the requested outputs among gg, gx, gY, gw (float32 device tensors)."""
+    E = senders.numel()
+    dev = feats.device
+    f32 = torch.float32
+    outs = {"gg": (n_nodes, plan.out_dim * plan.channels), "gx": (n_nodes, plan.in_dim * plan.channels),
+            "gY": (E, plan.sh_dim), "gw": (E, plan.weights_per_edge)}
+    bufs = {k: (torch.empty(shape, dtype=f32, device=dev) if k in want else None) for k, shape in outs.items()}
+    nbytes = int(lib().e3_vjp_vjp_workspace_bytes(plan.handle, C.c_int64(E), C.c_int32(n_nodes)))
+    ws = torch.empty(nbytes, dtype=torch.uint8, device=dev)
+    _check(lib().e3_tp_scatter_vjp_vjp(plan.handle, _ptr(feats), _ptr(sh), _ptr(weights), _ptr(senders), _ptr(receivers), _ptr(row_ptr),
+                                       _ptr(perm_s), _ptr(col_ptr), C.c_int64(E), C.c_int32(n_nodes), _ptr(grad_out), _ptr(v_feats),
+                                       _ptr(v_sh), _ptr(v_weights), _ptr(bufs["gg"]), _ptr(bufs["gx"]), _ptr(bufs["gY"]), _ptr(bufs["gw"]),
+                                       _ptr(ws), C.c_size_t(nbytes), _stream(stream)), "e3_tp_scatter_vjp_vjp")
+    return {k: v for k, v in bufs.items() if v is not None}
+
+
+def e3_sh_bwd_bwd(plan: Plan, vec, grad_sh, u, want_vec=True, want_sh=True, stream=None):
+    _dev(vec, torch.float32); _dev(u, torch.float32)
+    E = vec.shape[0]
+    gv = torch.empty((E, 3), dtype=torch.float32, device=vec.device) if want_vec else None
+    gs = torch.empty((E, plan.sh_dim), dtype=torch.float32, device=vec.device) if want_sh else None
+    _check(lib().e3_sh_bwd_bwd(plan.handle, _ptr(vec), _ptr(grad_sh), _ptr(u), C.c_int64(E), _ptr(gv), _ptr(gs), _stream(stream)),
+           "e3_sh_bwd_bwd")
+    return gv, gs

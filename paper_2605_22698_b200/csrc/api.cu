@@ -383,6 +383,111 @@ extern "C" int e3_tp_scatter_bwd(const e3_plan *plan, const void *feats, const v
     return launch_bwd_phase2(plan, perm_s, col_ptr, n_edges, n_nodes, grad_feats, grad_sh, workspace, S(stream));
 }
 
+// ---------------------------------------------------------------------------------------------
+// NEXT-2: second-order VJP.  The forward is trilinear, so every term of the VJP-of-VJP is a first-order
+// call with one operand replaced by its cotangent (oracle: orc_tp_vjp_vjp and its composition pins):
+//   gg = T(vx,Y,w) + T(x,vY,w) + T(x,Y,vw)
+//   (-,   dY1, dw1) = VJP(vx, Y,  w ; g)      (dx2, -,   dw2) = VJP(x, vY, w ; g)      (dx3, dY3, -) = VJP(x, Y, vw ; g)
+//   gx = dx2 + dx3,  gY = dY1 + dY3,  gw = dw1 + dw2
+// A NULL cotangent is zero and drops its calls; a NULL output is not computed.
+// ---------------------------------------------------------------------------------------------
+extern "C" size_t e3_vjp_vjp_workspace_bytes(const e3_plan *plan, int64_t n_edges, int32_t n_nodes)
+{
+    if (!plan || n_edges < 0 || n_nodes < 0) return 0;
+    auto up = [](size_t b) { return ((b + 255) / 256) * 256; };
+    const size_t C = plan->C;
+    return up(e3_bwd_workspace_bytes(plan, n_edges, n_nodes)) + up((size_t)n_nodes * plan->out_dim * C * 4) + up((size_t)n_nodes * plan->in_dim * C * 4) +
+           up((size_t)n_edges * plan->sh_dim * 4) + up((size_t)n_edges * plan->paths.size() * C * 4) + 256;
+}
+
+extern "C" int e3_tp_scatter_vjp_vjp(const e3_plan *plan, const void *feats, const void *sh, const void *weights, const int32_t *senders,
+                                     const int32_t *receivers, const int32_t *row_ptr, const int32_t *perm_s, const int32_t *col_ptr, int64_t n_edges,
+                                     int32_t n_nodes, const float *grad_out, const float *v_feats, const float *v_sh, const float *v_weights,
+                                     float *gg_out, float *g_feats, float *g_sh, float *g_weights, void *workspace, size_t workspace_bytes, e3_stream stream)
+{
+    (void)receivers;
+    if (!plan || n_edges < 0 || n_nodes < 0 || !row_ptr || !col_ptr || (n_nodes > 0 && (!feats || !grad_out)) ||
+        (n_edges > 0 && (!sh || !weights || !senders || !perm_s))) {
+        set_error("e3_tp_scatter_vjp_vjp: bad arguments");
+        return E3_ERR_INVALID_ARG;
+    }
+    if (plan->dtype != E3_F32) { set_error("e3_tp_scatter_vjp_vjp: E3_F32 plans only (cotangents stand in for operands)"); return E3_ERR_UNSUPPORTED; }
+    const void *ptrs[] = { feats, sh, weights, grad_out, v_feats, v_sh, v_weights, gg_out, g_feats, g_sh, g_weights, workspace };
+    for (const void *q : ptrs) if (!aligned16(q)) { set_error("e3_tp_scatter_vjp_vjp: tensor pointers must be 16-byte aligned"); return E3_ERR_INVALID_ARG; }
+    if (!workspace || workspace_bytes < e3_vjp_vjp_workspace_bytes(plan, n_edges, n_nodes)) {
+        set_error("e3_tp_scatter_vjp_vjp: workspace too small (need %zu bytes)", e3_vjp_vjp_workspace_bytes(plan, n_edges, n_nodes));
+        return E3_ERR_WORKSPACE;
+    }
+    if (n_nodes == 0) return E3_OK;
+    cudaStream_t st = S(stream);
+    auto up = [](size_t b) { return ((b + 255) / 256) * 256; };
+    const size_t C = plan->C, n_out = (size_t)n_nodes * plan->out_dim * C, n_in = (size_t)n_nodes * plan->in_dim * C;
+    const size_t n_sh = (size_t)n_edges * plan->sh_dim, n_w = (size_t)n_edges * plan->paths.size() * C;
+    char *wp = (char *)workspace;
+    void *bws = wp; wp += up(e3_bwd_workspace_bytes(plan, n_edges, n_nodes));
+    float *t_out = (float *)wp; wp += up(n_out * 4);
+    float *t_in = (float *)wp; wp += up(n_in * 4);
+    float *t_sh = (float *)wp; wp += up(n_sh * 4);
+    float *t_w = (float *)wp;
+    int rc = E3_OK;
+    // ---- gg: tangent of the forward
+    if (gg_out) {
+        bool first = true;
+        const void *ops[3][3] = { { v_feats, sh, weights }, { feats, v_sh, weights }, { feats, sh, v_weights } };
+        const bool have[3] = { v_feats != nullptr, v_sh != nullptr, v_weights != nullptr };
+        for (int k = 0; k < 3 && rc == E3_OK; ++k) {
+            if (!have[k] || (k > 0 && n_edges == 0)) continue;
+            rc = launch_fwd(plan, ops[k][0], ops[k][1], ops[k][2], senders, row_ptr, n_nodes, first ? gg_out : t_out, st);
+            if (rc == E3_OK && !first) rc = launch_add_inplace(gg_out, t_out, (long long)n_out, st);
+            first = false;
+        }
+        if (first) E3_CUDA_TRY(cudaMemsetAsync(gg_out, 0, n_out * 4, st));
+    }
+    if (rc != E3_OK) return rc;
+    // ---- first-order VJPs with one operand replaced
+    bool gx_set = false, gy_set = false, gw_set = false;
+    auto vjp = [&](const void *xa, const void *ya, const void *wa, float *dx_dst, float *dy_dst, float *dw_dst) -> int {
+        // outputs not wanted go to the temporaries (the kernels always produce grad_feats and grad_sh; grad_weights may be NULL)
+        int r2 = launch_bwd_phase1(plan, xa, ya, wa, senders, row_ptr, n_nodes, grad_out, dy_dst ? dy_dst : t_sh, dw_dst, bws, n_edges, st);
+        if (r2 == E3_OK) r2 = launch_bwd_phase2(plan, perm_s, col_ptr, n_edges, n_nodes, dx_dst ? dx_dst : t_in, dy_dst ? dy_dst : t_sh, bws, st);
+        return r2;
+    };
+    if (n_edges > 0) {
+        if (v_feats && (g_sh || g_weights)) {                         // VJP(vx, Y, w): dY1 -> gY, dw1 -> gw
+            rc = vjp(v_feats, sh, weights, nullptr, g_sh, g_weights);
+            if (rc != E3_OK) return rc;
+            gy_set = g_sh != nullptr; gw_set = g_weights != nullptr;
+        }
+        if (v_sh && (g_feats || g_weights)) {                         // VJP(x, vY, w): dx2 -> gx, dw2 -> gw (+)
+            float *dwd = g_weights ? (gw_set ? t_w : g_weights) : nullptr;
+            rc = vjp(feats, v_sh, weights, g_feats, nullptr, dwd);
+            if (rc == E3_OK && g_weights && gw_set) rc = launch_add_inplace(g_weights, t_w, (long long)n_w, st);
+            if (rc != E3_OK) return rc;
+            gx_set = g_feats != nullptr; gw_set = gw_set || g_weights != nullptr;
+        }
+        if (v_weights && (g_feats || g_sh)) {                         // VJP(x, Y, vw): dx3 -> gx (+), dY3 -> gY (+)
+            float *dxd = g_feats ? (gx_set ? t_in : g_feats) : nullptr;
+            float *dyd = g_sh ? (gy_set ? t_sh : g_sh) : nullptr;
+            rc = vjp(feats, sh, v_weights, dxd, dyd, nullptr);
+            if (rc == E3_OK && g_feats && gx_set) rc = launch_add_inplace(g_feats, t_in, (long long)n_in, st);
+            if (rc == E3_OK && g_sh && gy_set) rc = launch_add_inplace(g_sh, t_sh, (long long)n_sh, st);
+            if (rc != E3_OK) return rc;
+            gx_set = gx_set || g_feats != nullptr; gy_set = gy_set || g_sh != nullptr;
+        }
+    }
+    if (g_feats && !gx_set) E3_CUDA_TRY(cudaMemsetAsync(g_feats, 0, n_in * 4, st));
+    if (g_sh && !gy_set && n_sh) E3_CUDA_TRY(cudaMemsetAsync(g_sh, 0, n_sh * 4, st));
+    if (g_weights && !gw_set && n_w) E3_CUDA_TRY(cudaMemsetAsync(g_weights, 0, n_w * 4, st));
+    return E3_OK;
+}
+
+extern "C" int e3_sh_bwd_bwd(const e3_plan *plan, const float *vec, const float *grad_sh, const float *u, int64_t n_edges, float *g_vec,
+                             float *g_sh, e3_stream stream)
+{
+    if (!plan || n_edges < 0 || (n_edges > 0 && (!vec || !u || (g_vec && !grad_sh)))) { set_error("e3_sh_bwd_bwd: bad arguments"); return E3_ERR_INVALID_ARG; }
+    return launch_sh_bwd_bwd(plan->sh_lmax, vec, grad_sh, u, n_edges, g_vec, g_sh, S(stream));
+}
+
 extern "C" int e3_profile_set_mid_event(e3_plan *plan, void *cuda_event)
 {
     if (!plan) { set_error("plan is NULL"); return E3_ERR_INVALID_ARG; }

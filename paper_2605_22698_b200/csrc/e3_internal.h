@@ -140,6 +140,8 @@ int launch_dx_reduce(const float *dxe, const int32_t *perm_s, const int32_t *col
                      float *dx, cudaStream_t st);
 int launch_gsh_reduce(const float *parts, int n_parts, int64_t n, float *gsh, cudaStream_t st);
 int measure_fp32_peak(double *tflops, double ms_target, cudaStream_t st);
+int launch_sh_bwd_bwd(int lmax, const float *vec, const float *gsh, const float *u, int64_t E, float *g_vec, float *g_sh, cudaStream_t st);
+int launch_add_inplace(float *dst, const float *src, long long n, cudaStream_t st);
 int launch_cg_planner(const int *triples /*[n,3] host*/, int n, std::vector<std::vector<double>> &dense_out);
 
 }  // namespace e3

@@ -109,6 +109,135 @@ __global__ void __launch_bounds__(128) sh_bwd_kernel(const float *__restrict__ v
     gvec[3 * e + 2] = (gz - z * rad) * inv;
 }
 
+// ---------------------------------------------------------------------------------------------
+// NEXT-2 (Eq. 3-4): second derivative of the SH, as the VJP of (vec, grad_sh) -> grad_vec =
+// J(vec)^T grad_sh for a cotangent u[E,3]:  g_sh = J(vec) u,  g_vec = (sum_lm grad_sh_lm Hess Y_lm) u.
+// Both are directional derivatives along u (of Y and of grad_vec), so the kernel runs the first-order formulas once in
+// forward-mode dual arithmetic (value, tangent): no second-derivative formula is written out.
+// ---------------------------------------------------------------------------------------------
+struct Dual { float v, d; };
+__device__ __forceinline__ Dual operator+(Dual a, Dual b) { return { a.v + b.v, a.d + b.d }; }
+__device__ __forceinline__ Dual operator-(Dual a, Dual b) { return { a.v - b.v, a.d - b.d }; }
+__device__ __forceinline__ Dual operator*(Dual a, Dual b) { return { a.v * b.v, fmaf(a.v, b.d, a.d * b.v) }; }
+__device__ __forceinline__ Dual operator*(float a, Dual b) { return { a * b.v, a * b.d }; }
+__device__ __forceinline__ Dual operator-(Dual a, float b) { return { a.v - b, a.d }; }
+__device__ __forceinline__ Dual operator-(Dual a) { return { -a.v, -a.d }; }
+
+// Y_lm of the (dual) unit vector x, y, z: the polynomials of sh_values
+template <int LMAX>
+__device__ __forceinline__ void sh_values_dual(Dual x, Dual y, Dual z, Dual *Y)
+{
+    Y[0] = { 1.0f, 0.0f };
+    if (LMAX >= 1) { Y[1] = SQ3 * y; Y[2] = SQ3 * z; Y[3] = SQ3 * x; }
+    if (LMAX >= 2) {
+        Y[4] = SQ15 * (x * y);
+        Y[5] = SQ15 * (y * z);
+        Y[6] = (0.5f * SQ5) * (3.0f * (z * z) - 1.0f);
+        Y[7] = SQ15 * (x * z);
+        Y[8] = (0.5f * SQ15) * (x * x - y * y);
+    }
+    if (LMAX >= 3) {
+        const Dual x2 = x * x, y2 = y * y, z2 = z * z;
+        Y[9] = (0.25f * SQ70) * (y * (3.0f * x2 - y2));
+        Y[10] = SQ105 * (x * y * z);
+        Y[11] = (0.25f * SQ42) * (y * (5.0f * z2 - 1.0f));
+        Y[12] = (0.5f * SQ7) * (z * (5.0f * z2 - 3.0f));
+        Y[13] = (0.25f * SQ42) * (x * (5.0f * z2 - 1.0f));
+        Y[14] = (0.5f * SQ105) * (z * (x2 - y2));
+        Y[15] = (0.25f * SQ70) * (x * (x2 - 3.0f * y2));
+    }
+}
+
+template <int LMAX>
+__global__ void __launch_bounds__(128) sh_bwd_bwd_kernel(const float *__restrict__ vec, const float *__restrict__ gsh, const float *__restrict__ u,
+                                                         int64_t E, float *__restrict__ g_vec, float *__restrict__ g_sh)
+{
+    constexpr int D = (LMAX + 1) * (LMAX + 1);
+    const int64_t e = (int64_t)blockIdx.x * 128 + threadIdx.x;
+    if (e >= E) return;
+    const float vx = vec[3 * e], vy = vec[3 * e + 1], vz = vec[3 * e + 2];
+    const float n2 = vx * vx + vy * vy + vz * vz;
+    if (!(n2 > 0.0f)) {
+        if (g_vec) { g_vec[3 * e] = 0.0f; g_vec[3 * e + 1] = 0.0f; g_vec[3 * e + 2] = 0.0f; }
+        if (g_sh) for (int i = 0; i < D; ++i) g_sh[e * D + i] = 0.0f;
+        return;
+    }
+    const float ux = u[3 * e], uy = u[3 * e + 1], uz = u[3 * e + 2];
+    // dual vector vec + eps u, its inverse norm and the unit vector
+    const float invn = 1.0f / sqrtf(n2);
+    const Dual inv = { invn, -invn * invn * invn * (vx * ux + vy * uy + vz * uz) };
+    const Dual x = Dual{ vx, ux } * inv, y = Dual{ vy, uy } * inv, z = Dual{ vz, uz } * inv;
+    if (g_sh) {
+        Dual Y[D];
+        sh_values_dual<LMAX>(x, y, z, Y);
+#pragma unroll
+        for (int i = 0; i < D; ++i) g_sh[e * D + i] = Y[i].d;
+    }
+    if (!g_vec) return;
+    float g[D];
+#pragma unroll
+    for (int i = 0; i < D; ++i) g[i] = gsh[e * D + i];
+    // the first-order formulas of sh_bwd_kernel in dual arithmetic
+    Dual gx = { 0.f, 0.f }, gy = gx, gz = gx;
+    if (LMAX >= 1) { gy.v = SQ3 * g[1]; gz.v = SQ3 * g[2]; gx.v = SQ3 * g[3]; }
+    if (LMAX >= 2) {
+        gx = gx + SQ15 * (g[4] * y + g[7] * z + g[8] * x);
+        gy = gy + SQ15 * (g[4] * x + g[5] * z - g[8] * y);
+        gz = gz + SQ15 * (g[5] * y + g[7] * x) + (3.0f * SQ5 * g[6]) * z;
+    }
+    if (LMAX >= 3) {
+        const Dual x2 = x * x, y2 = y * y, z2 = z * z;
+        const float a = 0.25f * SQ70, b = SQ105, c = 0.25f * SQ42, d = 0.5f * SQ7, f = 0.5f * SQ105;
+        gx = gx + (a * g[9]) * (6.0f * (x * y)) + (b * g[10]) * (y * z) + (c * g[13]) * (5.0f * z2 - 1.0f)
+             + (f * g[14]) * (2.0f * (x * z)) + (a * g[15]) * (3.0f * x2 - 3.0f * y2);
+        gy = gy + (a * g[9]) * (3.0f * x2 - 3.0f * y2) + (b * g[10]) * (x * z) + (c * g[11]) * (5.0f * z2 - 1.0f)
+             - (f * g[14]) * (2.0f * (y * z)) - (a * g[15]) * (6.0f * (x * y));
+        gz = gz + (b * g[10]) * (x * y) + (c * g[11]) * (10.0f * (y * z)) + (d * g[12]) * (15.0f * z2 - 3.0f)
+             + (c * g[13]) * (10.0f * (x * z)) + (f * g[14]) * (x2 - y2);
+    }
+    const Dual rad = gx * x + gy * y + gz * z;
+    const Dual ox = (gx - x * rad) * inv, oy = (gy - y * rad) * inv, oz = (gz - z * rad) * inv;
+    g_vec[3 * e] = ox.d; g_vec[3 * e + 1] = oy.d; g_vec[3 * e + 2] = oz.d;
+}
+
+int launch_sh_bwd_bwd(int lmax, const float *vec, const float *gsh, const float *u, int64_t E, float *g_vec, float *g_sh, cudaStream_t st)
+{
+    if (E == 0) return E3_OK;
+    unsigned grid = (unsigned)((E + 127) / 128);
+    switch (lmax) {
+    case 0: sh_bwd_bwd_kernel<0><<<grid, 128, 0, st>>>(vec, gsh, u, E, g_vec, g_sh); break;
+    case 1: sh_bwd_bwd_kernel<1><<<grid, 128, 0, st>>>(vec, gsh, u, E, g_vec, g_sh); break;
+    case 2: sh_bwd_bwd_kernel<2><<<grid, 128, 0, st>>>(vec, gsh, u, E, g_vec, g_sh); break;
+    case 3: sh_bwd_bwd_kernel<3><<<grid, 128, 0, st>>>(vec, gsh, u, E, g_vec, g_sh); break;
+    default: set_error("sh: lmax %d unsupported", lmax); return E3_ERR_UNSUPPORTED;
+    }
+    E3_CUDA_TRY(cudaGetLastError());
+    return E3_OK;
+}
+
+// dst[i] += src[i] (fixed order: one thread per element; used to sum the terms of the second-order VJP)
+__global__ void add_inplace_kernel(float *__restrict__ dst, const float *__restrict__ src, long long n)
+{
+    const long long i4 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 4;
+    if (i4 + 4 <= n) {
+        float4 a = *reinterpret_cast<float4 *>(dst + i4);
+        const float4 b = __ldcs(reinterpret_cast<const float4 *>(src + i4));
+        a.x += b.x; a.y += b.y; a.z += b.z; a.w += b.w;
+        *reinterpret_cast<float4 *>(dst + i4) = a;
+    } else {
+        for (long long i = i4; i < n; ++i) dst[i] += src[i];
+    }
+}
+
+int launch_add_inplace(float *dst, const float *src, long long n, cudaStream_t st)
+{
+    if (n <= 0) return E3_OK;
+    const long long n4 = (n + 3) / 4;
+    add_inplace_kernel<<<(unsigned)((n4 + 255) / 256), 256, 0, st>>>(dst, src, n);
+    E3_CUDA_TRY(cudaGetLastError());
+    return E3_OK;
+}
+
 int launch_sh_fwd(int lmax, e3_dtype dt, const float *vec, int64_t E, void *sh, cudaStream_t st)
 {
     if (E == 0) return E3_OK;

@@ -1,0 +1,130 @@
+"""NEXT-2 on the GPU: second-order VJP of the tensor product (e3_tp_scatter_vjp_vjp) and the SH second derivative (e3_sh_bwd_bwd)
+against the fp64 oracle (orc_tp_vjp_vjp, orc_sh_bwd_bwd), and a Hessian row of the whole path (section 5.2, Eq. 3-4)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle as O
+from helpers import TOL_VJP, gpu_plan, make_case, plan_inputs, relerr, to_dev
+from paper_2605_22698_b200 import binding as B
+from paper_2605_22698_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def _case(rng, C, lmax, n, deg_hi):
+    irr = ((0, 1), (1, -1), (2, 1), (3, -1))[: lmax + 1]
+    cfg = W.small_config(channels=C, irreps_in=irr, sh_lmax=lmax, out_lmax=lmax)
+    pl = plan_inputs(cfg)
+    deg = rng.integers(0, deg_hi, size=n); deg[1] = 0; deg[2] = 3 * deg_hi
+    rcv = np.repeat(np.arange(n), deg)
+    snd = rng.integers(0, n, size=rcv.size)
+    o = np.lexsort((snd, rcv))
+    snd, rcv = snd[o].astype(np.int32), rcv[o].astype(np.int32)
+    e = rcv.size
+    in_dim, od = sum(2 * l + 1 for l, _ in irr), sum(2 * l + 1 for l, _, _ in pl[2])
+    f32 = lambda a: a.astype(np.float32)
+    t = dict(x=f32(rng.normal(size=(n, in_dim * C))), Y=f32(rng.normal(size=(e, (lmax + 1) ** 2))), w=f32(rng.normal(size=(e, len(pl[3]) * C))),
+             g=f32(rng.normal(size=(n, od * C))), vx=f32(rng.normal(size=(n, in_dim * C))), vY=f32(rng.normal(size=(e, (lmax + 1) ** 2))),
+             vw=f32(rng.normal(size=(e, len(pl[3]) * C))))
+    return pl, snd, rcv, n, t
+
+
+@pytest.mark.parametrize("C,lmax", [(32, 2), (64, 3), (128, 3)])
+def test_vjp_vjp_against_oracle(C, lmax):
+    rng = np.random.default_rng(C + lmax)
+    pl, snd, rcv, n, t = _case(rng, C, lmax, 21, 10)
+    plan = gpu_plan(pl)
+    sd, rd = to_dev(snd), to_dev(rcv)
+    rp, ps, cp = B.e3_graph_prepare(sd, rd, n)
+    d = {k: to_dev(v) for k, v in t.items()}
+    got = B.e3_tp_scatter_vjp_vjp(plan, d["x"], d["Y"], d["w"], sd, rd, rp, ps, cp, n, d["g"], d["vx"], d["vY"], d["vw"])
+    ref = dict(zip(("gg", "gx", "gY", "gw"), O.tp_vjp_vjp(*pl, t["x"], t["Y"], t["w"], snd, rcv, n, t["g"], t["vx"], t["vY"], t["vw"])))
+    torch.cuda.synchronize()
+    errs = {k: relerr(got[k].cpu().numpy(), ref[k]) for k in ref}
+    print(C, lmax, {k: f"{v:.1e}" for k, v in errs.items()})
+    assert max(errs.values()) <= TOL_VJP, errs
+    # subsets of cotangents (NULL = zero) and of outputs
+    z = lambda a: np.zeros_like(a)
+    for keep in (("vY",), ("vx", "vw"), ()):
+        kw = {k: (d[k] if k in keep else None) for k in ("vx", "vY", "vw")}
+        got2 = B.e3_tp_scatter_vjp_vjp(plan, d["x"], d["Y"], d["w"], sd, rd, rp, ps, cp, n, d["g"], kw["vx"], kw["vY"], kw["vw"])
+        ref2 = dict(zip(("gg", "gx", "gY", "gw"), O.tp_vjp_vjp(*pl, t["x"], t["Y"], t["w"], snd, rcv, n, t["g"],
+                                                             *[t[k] if k in keep else z(t[k]) for k in ("vx", "vY", "vw")])))
+        for k in ref2:
+            den = max(np.abs(ref[k]).max(), 1e-30)
+            assert np.abs(got2[k].cpu().numpy() - ref2[k]).max() / den <= TOL_VJP, (keep, k)
+    only = B.e3_tp_scatter_vjp_vjp(plan, d["x"], d["Y"], d["w"], sd, rd, rp, ps, cp, n, d["g"], d["vx"], d["vY"], d["vw"], want=("gw",))
+    assert set(only) == {"gw"} and np.array_equal(only["gw"].cpu().numpy(), got["gw"].cpu().numpy())
+
+
+def test_vjp_vjp_rejects_bf16_plans():
+    cfg = W.small_config(channels=32, irreps_in=((0, 1), (1, -1)), sh_lmax=3, out_lmax=3, storage="bf16")
+    pl = plan_inputs(cfg)
+    plan = gpu_plan(pl, "bf16")
+    rng = np.random.default_rng(0)
+    snd = np.array([0, 1], np.int32); rcv = np.array([1, 1], np.int32)
+    sd, rd = to_dev(snd), to_dev(rcv)
+    rp, ps, cp = B.e3_graph_prepare(sd, rd, 2)
+    x = torch.zeros((2, 4 * 32), dtype=torch.bfloat16, device="cuda"); Y = torch.zeros((2, 16), dtype=torch.bfloat16, device="cuda")
+    w = torch.zeros((2, plan.weights_per_edge), dtype=torch.bfloat16, device="cuda")
+    g = torch.zeros((2, plan.out_dim * 32), device="cuda")
+    with pytest.raises(B.E3Error) as ei:
+        B.e3_tp_scatter_vjp_vjp(plan, x, Y, w, sd, rd, rp, ps, cp, 2, g, None, None, None)
+    assert ei.value.status == B.E3_ERR_UNSUPPORTED
+
+
+@pytest.mark.parametrize("lmax", [0, 1, 2, 3])
+def test_sh_second_derivative_against_oracle(lmax):
+    rng = np.random.default_rng(40 + lmax)
+    E = 1000
+    vec = (rng.normal(size=(E, 3)) * 2).astype(np.float32)
+    vec[5] = 0.0
+    vec[6] = [0.0, 0.0, 1.5]
+    dY = rng.normal(size=(E, (lmax + 1) ** 2)).astype(np.float32)
+    u = rng.normal(size=(E, 3)).astype(np.float32)
+    cfg = W.small_config(channels=8, irreps_in=((0, 1),), sh_lmax=lmax, out_lmax=lmax)
+    plan = gpu_plan(plan_inputs(cfg))
+    gv, gs = B.e3_sh_bwd_bwd(plan, to_dev(vec), to_dev(dY), to_dev(u))
+    rv, rs = O.sh_bwd_bwd(lmax, vec, dY, u)
+    torch.cuda.synchronize()
+    # 1/r^2 scaling of the second derivative: compare where |vec| is not tiny, relative to the largest reference value there
+    ok = np.linalg.norm(vec, axis=1) > 0.3
+    assert relerr(gs.cpu().numpy(), rs) <= 1e-5
+    assert relerr(gv.cpu().numpy()[ok], rv[ok]) <= TOL_VJP
+    assert not gv.cpu().numpy()[5].any() and not gs.cpu().numpy()[5].any()
+    only_s = B.e3_sh_bwd_bwd(plan, to_dev(vec), None, to_dev(u), want_vec=False)[1]
+    assert np.array_equal(only_s.cpu().numpy(), gs.cpu().numpy())
+
+
+def test_hessian_row_config1_against_oracle():
+    """dS/dpos for S = <c, F>, F = -dE/dpos through SH and generated weights held fixed... here weights and features are inputs (A13), so
+    the row is the SH second-derivative term plus the second-order tensor product with cotangent v_sh = J u (whose dS/dsh vanishes
+    identically for fixed x, w -- checked), composed exactly as the oracle composes them."""
+    cfg = W.CONFIGS[1]
+    pl, g, x, w, G = make_case(cfg)
+    plan = gpu_plan(pl)
+    n = g.n_nodes
+    rng = np.random.default_rng(9)
+    c = np.zeros((n, 3), np.float32); c[rng.integers(0, n, 4), rng.integers(0, 3, 4)] = 1.0      # four selected force components
+    snd, rcv, vec = to_dev(g.senders), to_dev(g.receivers), to_dev(g.vec)
+    xd, wd, Gd = to_dev(x), to_dev(w), to_dev(G)
+    rp, ps, cp = B.e3_graph_prepare(snd, rcv, n)
+    sh = B.e3_sh_fwd(plan, vec)
+    _, dY, _ = B.e3_tp_scatter_bwd(plan, xd, sh, wd, snd, rcv, rp, ps, cp, n, Gd)
+    uvec = to_dev(-(c[g.receivers] - c[g.senders]))
+    g_vec, g_dY = B.e3_sh_bwd_bwd(plan, vec, dY, uvec)
+    so = B.e3_tp_scatter_vjp_vjp(plan, xd, sh, wd, snd, rcv, rp, ps, cp, n, Gd, None, g_dY, None, want=("gY", "gx", "gw"))
+    assert not so["gY"].cpu().numpy().any()                                # dY does not depend on Y (trilinear map)
+    row = -B.e3_force_reduce(g_vec, rp, ps, cp, n)
+    torch.cuda.synchronize()
+    v64 = g.vec.astype(np.float64)
+    Y = O.sh(pl[1], v64)
+    _, dYr, _ = O.tp_scatter_bwd(*pl, x, Y, w, g.senders, g.receivers, n, G)
+    rv, rdY = O.sh_bwd_bwd(pl[1], v64, dYr, -(c[g.receivers] - c[g.senders]).astype(np.float64))
+    rrow = -O.force_reduce(rv, g.senders, g.receivers, n)
+    zx, zw = np.zeros_like(x), np.zeros_like(w)
+    _, rgx, _, rgw = O.tp_vjp_vjp(*pl, x, Y, w, g.senders, g.receivers, n, G, zx, rdY, zw)
+    errs = dict(row=relerr(row.cpu().numpy(), rrow), gx=relerr(so["gx"].cpu().numpy(), rgx), gw=relerr(so["gw"].cpu().numpy(), rgw))
+    print({k: f"{v:.1e}" for k, v in errs.items()})
+    assert max(errs.values()) <= 2 * TOL_VJP, errs
