@@ -325,3 +325,59 @@ def sh_bwd_bwd(lmax, vec, dY, u):
     if rc:
         raise ValueError("lmax out of range")
     return gv, gd
+
+
+# --------------------------------------------------------------------------------------------
+# NEXT-3: symmetric contraction at correlation 2 (e3_oracle_next.c, reading S1)
+# --------------------------------------------------------------------------------------------
+def symcon_paths(irreps_in, out_lmax, natural_parity_only=True):
+    """Path table of the contraction: one linear path per input irrep with l <= out_lmax (its own output block) and one quadratic
+    path per (i1 <= i2, L) allowed by the triangle rule, output parity p1*p2 (natural parity (-1)^L only, unless told otherwise);
+    order: linear paths first (by i_in), then i1, i2, L ascending; each path gets its own output irrep.  Returns (irreps_out, paths)
+    with paths as (i_in1, i_in2 or -1, i_out)."""
+    irreps_out, paths = [], []
+    for i, (l, p, mul) in enumerate(irreps_in):
+        if l <= out_lmax:
+            irreps_out.append((l, p, mul)); paths.append((i, -1, len(irreps_out) - 1))
+    for i1, (l1, p1, mul) in enumerate(irreps_in):
+        for i2 in range(i1, len(irreps_in)):
+            l2, p2, _ = irreps_in[i2]
+            for L in range(abs(l1 - l2), min(l1 + l2, out_lmax) + 1):
+                if natural_parity_only and p1 * p2 != (-1) ** L:
+                    continue
+                irreps_out.append((L, p1 * p2, mul)); paths.append((i1, i2, len(irreps_out) - 1))
+    return irreps_out, paths
+
+
+class _ScPath(C.Structure):
+    _fields_ = [("i_in1", C.c_int), ("i_in2", C.c_int), ("i_out", C.c_int)]
+
+
+def _sc_args(irreps_in, irreps_out, paths, n_species):
+    ii = (_Irrep * len(irreps_in))(*[_Irrep(*map(int, t)) for t in irreps_in])
+    io = (_Irrep * len(irreps_out))(*[_Irrep(*map(int, t)) for t in irreps_out])
+    pp = (_ScPath * len(paths))(*[_ScPath(*map(int, t)) for t in paths])
+    return (ii, C.c_int(len(irreps_in)), io, C.c_int(len(irreps_out)), pp, C.c_int(len(paths)), C.c_int(int(n_species)))
+
+
+def symcon2_fwd(irreps_in, irreps_out, paths, n_species, A, species, W):
+    A, W, species = _f64(A), _f64(W), _i32(species)
+    N = A.shape[0]
+    Cm = int(irreps_in[0][2])
+    out_dim = sum(2 * l + 1 for l, _, _ in irreps_out)
+    assert W.shape == (n_species, len(paths), Cm)
+    B = np.empty((N, out_dim * Cm))
+    rc = _L().orc_symcon2_fwd(*_sc_args(irreps_in, irreps_out, paths, n_species), _p(A), _p(species), _p(W), C.c_int32(N), _p(B))
+    if rc:
+        raise ValueError(f"oracle symmetric contraction invalid (code {rc})")
+    return B
+
+
+def symcon2_bwd(irreps_in, irreps_out, paths, n_species, A, species, W, g):
+    A, W, g, species = _f64(A), _f64(W), _f64(g), _i32(species)
+    N = A.shape[0]
+    dA, dW = np.empty_like(A), np.empty_like(W)
+    rc = _L().orc_symcon2_bwd(*_sc_args(irreps_in, irreps_out, paths, n_species), _p(A), _p(species), _p(W), C.c_int32(N), _p(g), _p(dA), _p(dW))
+    if rc:
+        raise ValueError(f"oracle symmetric contraction invalid (code {rc})")
+    return dA, dW

@@ -389,3 +389,119 @@ int orc_sh_bwd_bwd(int lmax, int64_t n, const double *vec, const double *dY, con
     }
     return 0;
 }
+
+/* =================================================================================================================
+ * NEXT-3: MACE's symmetric contraction at correlation order 2 on node features (PAPER.md L535 `node_symmetry 2`, L536
+ * `correlation 2`, L545 `symmetric_contraction_backend e3j`; the paper prints no formula).  Reading S1: for node n of
+ * species z_n, channel u, every path carries one weight per species and channel, W[z, path, u]; a path is either
+ *   linear     (i_in1, -1,    i_out):  B[n, i_out, M, u] += W * A[n, i_in1, M, u]                      (correlation 1; same l and parity)
+ *   quadratic  (i_in1, i_in2, i_out):  B[n, i_out, M, u] += W * sum_{m1,m2} C^{l1 l2 L}[m1,m2,M] A[n,i_in1,m1,u] A[n,i_in2,m2,u]
+ * with the real CG tensors of reading A4 (triangle rule, parity p1*p2 = p_out).  Layout as everywhere (A7): block after block,
+ * index m*C + u.  All irreps share one multiplicity C.
+ * Pins (tests/test_oracle_next.py): brute-force einsum; Wigner-D equivariance and inversion; L = 0 closed form
+ * (-1)^l/sqrt(2l+1) |A_l|^2; the antisymmetric 1x1->1 self-product vanishes; VJP vs central differences and Euler's identity
+ * (the map is linear + quadratic in A).
+ * ================================================================================================================= */
+typedef struct { int i_in1; int i_in2; int i_out; } sc_path;
+
+static int sc_offsets(const nx_irrep *ir, int n, int *off) { int o = 0; for (int i = 0; i < n; ++i) { off[i] = o; o += 2 * ir[i].l + 1; } return o; }
+
+static int sc_check(const nx_irrep *ii, int n_in, const nx_irrep *io, int n_out, const sc_path *paths, int n_paths)
+{
+    if (n_in < 1 || n_out < 1 || n_paths < 1 || n_in > 64 || n_out > 64) return 1;
+    const int C = ii[0].mul;
+    for (int i = 0; i < n_in; ++i) if (ii[i].mul != C) return 2;
+    for (int i = 0; i < n_out; ++i) if (io[i].mul != C) return 2;
+    for (int p = 0; p < n_paths; ++p) {
+        const sc_path q = paths[p];
+        if (q.i_in1 < 0 || q.i_in1 >= n_in || q.i_in2 >= n_in || q.i_out < 0 || q.i_out >= n_out) return 3;
+        if (q.i_in2 < 0) {
+            if (ii[q.i_in1].l != io[q.i_out].l || ii[q.i_in1].parity != io[q.i_out].parity) return 4;
+        } else {
+            const int l1 = ii[q.i_in1].l, l2 = ii[q.i_in2].l, L = io[q.i_out].l;
+            if (L < abs(l1 - l2) || L > l1 + l2) return 4;
+            if (ii[q.i_in1].parity * ii[q.i_in2].parity != io[q.i_out].parity) return 5;
+        }
+    }
+    return 0;
+}
+
+int orc_symcon2_fwd(const nx_irrep *ii, int n_in, const nx_irrep *io, int n_out, const sc_path *paths, int n_paths, int n_species,
+                    const double *A, const int32_t *species, const double *W, int32_t N, double *B)
+{
+    int rc = sc_check(ii, n_in, io, n_out, paths, n_paths);
+    if (rc) return rc;
+    int in_off[64], out_off[64];
+    const int in_dim = sc_offsets(ii, n_in, in_off), out_dim = sc_offsets(io, n_out, out_off), C = ii[0].mul;
+    memset(B, 0, sizeof(double) * (size_t)N * out_dim * C);
+    for (int p = 0; p < n_paths; ++p) {
+        const sc_path q = paths[p];
+        const int L = io[q.i_out].l;
+        double *cg = NULL;
+        int l1 = ii[q.i_in1].l, l2 = 0;
+        if (q.i_in2 >= 0) { l2 = ii[q.i_in2].l; cg = (double *)malloc(sizeof(double) * (size_t)((2 * l1 + 1) * (2 * l2 + 1) * (2 * L + 1))); orc_cg_real(l1, l2, L, cg); }
+        for (int32_t n = 0; n < N; ++n) {
+            if (species[n] < 0 || species[n] >= n_species) { free(cg); return 6; }
+            const double *a = A + (int64_t)n * in_dim * C, *w = W + ((int64_t)species[n] * n_paths + p) * C;
+            double *b = B + (int64_t)n * out_dim * C;
+            for (int u = 0; u < C; ++u) {
+                if (q.i_in2 < 0) {
+                    for (int M = 0; M <= 2 * L; ++M) b[(out_off[q.i_out] + M) * C + u] += w[u] * a[(in_off[q.i_in1] + M) * C + u];
+                } else {
+                    for (int m1 = 0; m1 <= 2 * l1; ++m1)
+                        for (int m2 = 0; m2 <= 2 * l2; ++m2)
+                            for (int M = 0; M <= 2 * L; ++M)
+                                b[(out_off[q.i_out] + M) * C + u] += w[u] * cg[(m1 * (2 * l2 + 1) + m2) * (2 * L + 1) + M] *
+                                                                     a[(in_off[q.i_in1] + m1) * C + u] * a[(in_off[q.i_in2] + m2) * C + u];
+                }
+            }
+        }
+        free(cg);
+    }
+    return 0;
+}
+
+/* VJP: dA[N,in_dim*C] and dW[S,n_paths,C] (summed over the nodes of each species in ascending node order) for a cotangent g = dL/dB */
+int orc_symcon2_bwd(const nx_irrep *ii, int n_in, const nx_irrep *io, int n_out, const sc_path *paths, int n_paths, int n_species,
+                    const double *A, const int32_t *species, const double *W, int32_t N, const double *g, double *dA, double *dW)
+{
+    int rc = sc_check(ii, n_in, io, n_out, paths, n_paths);
+    if (rc) return rc;
+    int in_off[64], out_off[64];
+    const int in_dim = sc_offsets(ii, n_in, in_off), out_dim = sc_offsets(io, n_out, out_off), C = ii[0].mul;
+    memset(dA, 0, sizeof(double) * (size_t)N * in_dim * C);
+    memset(dW, 0, sizeof(double) * (size_t)n_species * n_paths * C);
+    for (int p = 0; p < n_paths; ++p) {
+        const sc_path q = paths[p];
+        const int L = io[q.i_out].l;
+        double *cg = NULL;
+        int l1 = ii[q.i_in1].l, l2 = 0;
+        if (q.i_in2 >= 0) { l2 = ii[q.i_in2].l; cg = (double *)malloc(sizeof(double) * (size_t)((2 * l1 + 1) * (2 * l2 + 1) * (2 * L + 1))); orc_cg_real(l1, l2, L, cg); }
+        for (int32_t n = 0; n < N; ++n) {
+            if (species[n] < 0 || species[n] >= n_species) { free(cg); return 6; }
+            const double *a = A + (int64_t)n * in_dim * C, *w = W + ((int64_t)species[n] * n_paths + p) * C, *gn = g + (int64_t)n * out_dim * C;
+            double *da = dA + (int64_t)n * in_dim * C, *dw = dW + ((int64_t)species[n] * n_paths + p) * C;
+            for (int u = 0; u < C; ++u) {
+                if (q.i_in2 < 0) {
+                    for (int M = 0; M <= 2 * L; ++M) {
+                        const double gv = gn[(out_off[q.i_out] + M) * C + u];
+                        da[(in_off[q.i_in1] + M) * C + u] += w[u] * gv;
+                        dw[u] += a[(in_off[q.i_in1] + M) * C + u] * gv;
+                    }
+                } else {
+                    for (int m1 = 0; m1 <= 2 * l1; ++m1)
+                        for (int m2 = 0; m2 <= 2 * l2; ++m2)
+                            for (int M = 0; M <= 2 * L; ++M) {
+                                const double c = cg[(m1 * (2 * l2 + 1) + m2) * (2 * L + 1) + M], gv = gn[(out_off[q.i_out] + M) * C + u];
+                                const double a1 = a[(in_off[q.i_in1] + m1) * C + u], a2 = a[(in_off[q.i_in2] + m2) * C + u];
+                                da[(in_off[q.i_in1] + m1) * C + u] += w[u] * c * a2 * gv;
+                                da[(in_off[q.i_in2] + m2) * C + u] += w[u] * c * a1 * gv;
+                                dw[u] += c * a1 * a2 * gv;
+                            }
+                }
+            }
+        }
+        free(cg);
+    }
+    return 0;
+}

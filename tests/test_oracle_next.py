@@ -198,3 +198,77 @@ def test_hessian_row_of_the_whole_path_against_finite_differences_of_forces():
             pp, pm = pos.copy(), pos.copy(); pp[i, a] += h; pm[i, a] -= h
             fd = ((c * forces(pp)).sum() - (c * forces(pm)).sum()) / (2 * h)
             assert abs(fd - dS_dpos[i, a]) < 2e-6 * max(1.0, np.abs(dS_dpos).max()), (i, a, fd, dS_dpos[i, a])
+
+
+# ------------------------------------------------------------------ NEXT-3: symmetric contraction, correlation 2
+def _wigner_from_sh(l, R, rng):
+    """Real Wigner-D of degree l obtained from the (pinned) SH alone: least squares of Y_l(R r) = D Y_l(r)."""
+    v = rng.normal(size=(6 * (2 * l + 1), 3))
+    Ya = O.sh(l, v)[:, l * l:(l + 1) ** 2]; Yb = O.sh(l, v @ R.T)[:, l * l:(l + 1) ** 2]
+    return np.linalg.lstsq(Ya, Yb, rcond=None)[0].T
+
+
+def test_symmetric_contraction_oracle():
+    rng = np.random.default_rng(21)
+    C, S = 3, 4
+    irreps_in = [(0, 1, C), (1, -1, C), (2, 1, C)]
+    irreps_out, paths = O.symcon_paths(irreps_in, 2)
+    assert [p for p in paths if p[1] < 0] == [(0, -1, 0), (1, -1, 1), (2, -1, 2)]
+    # quadratic, natural parity: (0,0,0) (0,1,1) (0,2,2) (1,1,0) (1,1,2) (1,2,1) (2,2,0) (2,2,2)   [(1,1,1), (1,2,2), (2,2,1) are pseudo-tensors]
+    assert [(irreps_in[a][0], irreps_in[b][0], irreps_out[o][0]) for a, b, o in paths if b >= 0] == \
+        [(0, 0, 0), (0, 1, 1), (0, 2, 2), (1, 1, 0), (1, 1, 2), (1, 2, 1), (2, 2, 0), (2, 2, 2)]
+    N = 7
+    A = rng.normal(size=(N, 9 * C)); z = rng.integers(0, S, size=N).astype(np.int32); W = rng.normal(size=(S, len(paths), C))
+    B = O.symcon2_fwd(irreps_in, irreps_out, paths, S, A, z, W)
+    # brute force with einsum
+    in_off = np.concatenate([[0], np.cumsum([2 * l + 1 for l, _, _ in irreps_in])])
+    out_off = np.concatenate([[0], np.cumsum([2 * l + 1 for l, _, _ in irreps_out])])
+    blk = lambda i: A[:, in_off[i] * C:in_off[i + 1] * C].reshape(N, -1, C)
+    ref = np.zeros_like(B)
+    for k, (a, b, o) in enumerate(paths):
+        dst = ref[:, out_off[o] * C:out_off[o + 1] * C].reshape(N, -1, C)
+        if b < 0:
+            dst += W[z, k][:, None, :] * blk(a)
+        else:
+            Cg = O.cg_real(irreps_in[a][0], irreps_in[b][0], irreps_out[o][0])
+            dst += W[z, k][:, None, :] * np.einsum("abc,nau,nbu->ncu", Cg, blk(a), blk(b))
+    assert np.abs(B - ref).max() < 1e-12
+    # L = 0 closed form: C(l,l,0) = (-1)^l delta / sqrt(2l+1)  =>  W * (-1)^l |A_l|^2 / sqrt(2l+1)
+    for k, (a, b, o) in enumerate(paths):
+        if b == a and irreps_out[o][0] == 0:
+            l = irreps_in[a][0]
+            want = W[z, k] * ((-1) ** l / np.sqrt(2 * l + 1)) * (blk(a) ** 2).sum(1)
+            only = np.zeros_like(W); only[:, k] = W[:, k]
+            got = O.symcon2_fwd(irreps_in, irreps_out, paths, S, A, z, only)[:, out_off[o] * C:out_off[o + 1] * C]
+            assert np.abs(got - want).max() < 1e-12
+    # the antisymmetric self-product 1 x 1 -> 1 vanishes identically
+    io2, p2 = O.symcon_paths([(1, -1, C)], 1, natural_parity_only=False)
+    k11 = [k for k, (a, b, o) in enumerate(p2) if b == 0 and io2[o][0] == 1][0]
+    W2 = np.zeros((S, len(p2), C)); W2[:, k11] = 1.0
+    assert np.abs(O.symcon2_fwd([(1, -1, C)], io2, p2, S, A[:, C:4 * C], z, W2)).max() < 1e-13
+    # equivariance: rotate every input block with its Wigner-D, outputs rotate with theirs; inversion flips odd blocks
+    q, _ = np.linalg.qr(rng.normal(size=(3, 3)))
+    if np.linalg.det(q) < 0:
+        q[:, 0] *= -1
+    D = {l: _wigner_from_sh(l, q, rng) for l in range(3)}
+    rot = lambda X, irreps: np.concatenate([np.einsum("ab,nbu->nau", D[l], X[:, o * C:(o + 2 * l + 1) * C].reshape(N, 2 * l + 1, C)).reshape(N, -1)
+                                           for (l, _, _), o in zip(irreps, np.concatenate([[0], np.cumsum([2 * t[0] + 1 for t in irreps])]))], axis=1)
+    assert np.abs(O.symcon2_fwd(irreps_in, irreps_out, paths, S, rot(A, irreps_in), z, W) - rot(B, irreps_out)).max() < 1e-11
+    par = lambda X, irreps: np.concatenate([p * X[:, o * C:(o + 2 * l + 1) * C] for (l, p, _), o in
+                                            zip(irreps, np.concatenate([[0], np.cumsum([2 * t[0] + 1 for t in irreps])]))], axis=1)
+    assert np.abs(O.symcon2_fwd(irreps_in, irreps_out, paths, S, par(A, irreps_in), z, W) - par(B, irreps_out)).max() < 1e-12
+    # VJP: central differences in A and W; dW only touches the rows of species present
+    g = rng.normal(size=B.shape)
+    dA, dW = O.symcon2_bwd(irreps_in, irreps_out, paths, S, A, z, W, g)
+    Lf = lambda A_, W_: float((g * O.symcon2_fwd(irreps_in, irreps_out, paths, S, A_, z, W_)).sum())
+    h = 1e-6
+    for arr, grad, k in ((A, dA, 0), (W, dW, 1)):
+        for _ in range(15):
+            idx = tuple(rng.integers(0, s) for s in arr.shape)
+            ap, am = arr.copy(), arr.copy(); ap[idx] += h; am[idx] -= h
+            args_p, args_m = [A, W], [A, W]
+            args_p[k], args_m[k] = ap, am
+            assert abs((Lf(*args_p) - Lf(*args_m)) / (2 * h) - grad[idx]) < 2e-7 * max(1.0, abs(grad[idx]))
+    assert abs((dW * W).sum() - (g * B).sum()) < 1e-10                     # linear in W: Euler identity
+    with pytest.raises(ValueError):
+        O.symcon2_fwd(irreps_in, [(3, -1, C)], [(0, 0, 0)], S, A, z, np.zeros((S, 1, C)))       # 0 x 0 -> 3 violates the triangle rule
