@@ -255,6 +255,33 @@ int e3_tp_scatter_vjp_vjp(const e3_plan *plan, const void *feats, const void *sh
 int e3_sh_bwd_bwd(const e3_plan *plan, const float *vec, const float *grad_sh, const float *u, int64_t n_edges,
                   float *g_vec, float *g_sh, e3_stream stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * NEXT-3: MACE's symmetric contraction at correlation order 2 on node features, the other operation the paper
+ * routes to e3j.  PAPER.md L535 (`node_symmetry 2`), L536 (`correlation 2`), L545 (`symmetric_contraction_backend e3j`); no
+ * formula is printed, so reading S1: for node n of species z = species[n] and channel u, every path k has the weight
+ * weights[(z*n_paths + k)*C + u] and is
+ *   linear     (i_in1, i_in2 = -1, i_out):  out[n, i_out, M, u] += W * feats[n, i_in1, M, u]              (same l and parity)
+ *   quadratic  (i_in1, i_in2,      i_out):  out[n, i_out, M, u] += W * sum_{m1,m2} C[m1,m2,M] feats[n,i_in1,m1,u] feats[n,i_in2,m2,u]
+ * with the real Clebsch-Gordan tensor C^{l1 l2 L} of reading A4 (triangle rule; parity p1*p2 = p_out; E3_ERR_BAD_PATH otherwise).
+ * Layout A7 (blocks concatenated, index m*C + u); all multiplicities equal; float tensors on the device; species int32 in
+ * [0, n_species) (values outside are clamped, never read out of bounds).  e3_symcon_bwd returns grad_feats [N,in_dim*C] and
+ * grad_weights [n_species,n_paths,C] (either may be NULL) for grad_out = dL/d out; workspace >= e3_symcon_workspace_bytes is needed
+ * for grad_weights.  Deterministic (every element is summed by one thread in a fixed order; grad_weights over 64 node chunks in
+ * chunk order).  e3_symcon_create needs a device (the CG tensors come from the planner kernel) and synchronises.
+ * -------------------------------------------------------------------------------------------*/
+typedef struct e3_symcon e3_symcon;
+typedef struct { int i_in1; int i_in2; int i_out; } e3_pair_path;
+int e3_symcon_create(e3_symcon **sc, const e3_irrep *irreps_in, int n_in, const e3_irrep *irreps_out, int n_out,
+                     const e3_pair_path *paths, int n_paths, int n_species);
+int e3_symcon_destroy(e3_symcon *sc);
+int e3_symcon_dims(const e3_symcon *sc, int *in_dim, int *out_dim, int *n_paths, int *n_terms);
+int e3_symcon_fwd(const e3_symcon *sc, const float *feats, const int32_t *species, const float *weights, int32_t n_nodes,
+                  float *out, e3_stream stream);
+size_t e3_symcon_workspace_bytes(const e3_symcon *sc, int32_t n_nodes);
+int e3_symcon_bwd(const e3_symcon *sc, const float *feats, const int32_t *species, const float *weights, int32_t n_nodes,
+                  const float *grad_out, float *grad_feats, float *grad_weights, void *workspace, size_t workspace_bytes,
+                  e3_stream stream);
+
 #ifdef __cplusplus
 }
 #endif

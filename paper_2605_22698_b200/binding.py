@@ -24,6 +24,7 @@ SYMBOLS = [
     "e3_graph_prepare", "e3_sh_fwd", "e3_sh_bwd", "e3_tp_scatter_fwd", "e3_bwd_workspace_bytes", "e3_tp_scatter_bwd",
     "e3_force_reduce", "e3_profile_set_mid_event", "e3_measure_fp32_peak", "e3_session_create", "e3_session_destroy", "e3_session_run_host",
     "e3_vjp_vjp_workspace_bytes", "e3_tp_scatter_vjp_vjp", "e3_sh_bwd_bwd",
+    "e3_symcon_create", "e3_symcon_destroy", "e3_symcon_dims", "e3_symcon_fwd", "e3_symcon_workspace_bytes", "e3_symcon_bwd",
     "e3_radial_create", "e3_radial_destroy", "e3_radial_workspace_bytes", "e3_radial_weights_fwd", "e3_radial_weights_bwd",
 ]
 
@@ -60,6 +61,8 @@ def lib():
         L.e3_bwd_workspace_bytes.argtypes = [C.c_void_p, C.c_int64, C.c_int32]
         L.e3_vjp_vjp_workspace_bytes.restype = C.c_size_t
         L.e3_vjp_vjp_workspace_bytes.argtypes = [C.c_void_p, C.c_int64, C.c_int32]
+        L.e3_symcon_workspace_bytes.restype = C.c_size_t
+        L.e3_symcon_workspace_bytes.argtypes = [C.c_void_p, C.c_int32]
         L.e3_radial_workspace_bytes.restype = C.c_size_t
         L.e3_radial_workspace_bytes.argtypes = [C.c_void_p, C.c_int64]
         _lib = L
@@ -367,3 +370,50 @@ def e3_sh_bwd_bwd(plan: Plan, vec, grad_sh, u, want_vec=True, want_sh=True, stre
     _check(lib().e3_sh_bwd_bwd(plan.handle, _ptr(vec), _ptr(grad_sh), _ptr(u), C.c_int64(E), _ptr(gv), _ptr(gs), _stream(stream)),
            "e3_sh_bwd_bwd")
     return gv, gs
+
+
+class _PairPath(C.Structure):
+    _fields_ = [("i_in1", C.c_int), ("i_in2", C.c_int), ("i_out", C.c_int)]
+
+
+class SymCon:
+    """Owns an ``e3_symcon*`` (NEXT-3: symmetric contraction at correlation 2).  paths: (i_in1, i_in2 or -1, i_out)."""
+
+    def __init__(self, irreps_in, irreps_out, paths, n_species):
+        self.handle = C.c_void_p()
+        pp = (_PairPath * len(paths))(*[_PairPath(*map(int, t)) for t in paths])
+        _check(lib().e3_symcon_create(C.byref(self.handle), _irreps(irreps_in), len(irreps_in), _irreps(irreps_out), len(irreps_out),
+                                      pp, len(paths), int(n_species)), "e3_symcon_create")
+        v = [C.c_int() for _ in range(4)]
+        _check(lib().e3_symcon_dims(self.handle, *[C.byref(t) for t in v]), "e3_symcon_dims")
+        self.in_dim, self.out_dim, self.n_paths, self.n_terms = [t.value for t in v]
+        self.channels, self.n_species = int(irreps_in[0][2]), int(n_species)
+
+    def fwd(self, feats, species, weights, stream=None):
+        _dev(feats, torch.float32); _dev(species, torch.int32); _dev(weights, torch.float32)
+        N = feats.shape[0]
+        out = torch.empty((N, self.out_dim * self.channels), dtype=torch.float32, device=feats.device)
+        _check(lib().e3_symcon_fwd(self.handle, _ptr(feats), _ptr(species), _ptr(weights), C.c_int32(N), _ptr(out), _stream(stream)), "e3_symcon_fwd")
+        return out
+
+    def bwd(self, feats, species, weights, grad_out, want_feats=True, want_weights=True, stream=None):
+        _dev(grad_out, torch.float32)
+        N = feats.shape[0]
+        dA = torch.empty_like(feats) if want_feats else None
+        dW = torch.empty_like(weights) if want_weights else None
+        nb = int(lib().e3_symcon_workspace_bytes(self.handle, C.c_int32(N)))
+        ws = torch.empty(nb, dtype=torch.uint8, device=feats.device)
+        _check(lib().e3_symcon_bwd(self.handle, _ptr(feats), _ptr(species), _ptr(weights), C.c_int32(N), _ptr(grad_out), _ptr(dA), _ptr(dW),
+                                   _ptr(ws), C.c_size_t(nb), _stream(stream)), "e3_symcon_bwd")
+        return dA, dW
+
+    def destroy(self):
+        if self.handle:
+            lib().e3_symcon_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

@@ -1,0 +1,305 @@
+// NEXT-3: MACE's symmetric contraction at correlation order 2 on node features, the other operation the paper routes
+// to e3j (PAPER.md L535 `node_symmetry 2`, L536 `correlation 2`, L545 `symmetric_contraction_backend e3j`).  The paper prints no
+// formula; reading S1: every path has one weight per species and channel, W[z, path, u], and is either
+//   linear     (i_in1, -1,    i_out):  B[n, i_out, M, u] += W * A[n, i_in1, M, u]
+//   quadratic  (i_in1, i_in2, i_out):  B[n, i_out, M, u] += W * sum_{m1,m2} C^{l1 l2 L}[m1,m2,M] A[n,i_in1,m1,u] A[n,i_in2,m2,u]
+// with the real Clebsch-Gordan tensors of reading A4 (computed by the device planner kernel of plan.cu).
+//
+// This is a per-node operation (N x C independent columns, no gather, no scatter): the kernels are table-driven.  The sparse CG
+// terms are flattened on the host into three CSR lists -- by OUTPUT row (forward), by INPUT row (grad_feats; a quadratic term
+// appears once for each of its two factors) and by PATH (grad_weights) -- so that every result element is accumulated in a
+// register by one thread in a fixed order (deterministic, no atomics).  A block owns one node and up to 128 channels; the node's
+// feature row (and cotangent row) is staged in shared memory.  grad_weights is a sum over the nodes of a species: per-chunk
+// partial sums (64 node chunks) written by one thread per (path, channel), added in chunk order by a second kernel.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <new>
+#include <vector>
+
+#include "e3_internal.h"
+
+using namespace e3;
+
+struct e3_symcon {
+    int n_in = 0, n_out = 0, n_paths = 0, n_species = 0, C = 0, in_dim = 0, out_dim = 0, nnz = 0;
+    // device tables
+    int *f_ptr = nullptr, *f_a1 = nullptr, *f_a2 = nullptr, *f_p = nullptr; float *f_c = nullptr;          // by output row
+    int *b_ptr = nullptr, *b_other = nullptr, *b_g = nullptr, *b_p = nullptr; float *b_c = nullptr;       // by input row
+    int *w_ptr = nullptr, *w_a1 = nullptr, *w_a2 = nullptr, *w_g = nullptr; float *w_c = nullptr;         // by path
+};
+
+namespace {
+
+constexpr int kChunks = 64;
+
+__global__ void symcon_fwd_kernel(const float *__restrict__ A, const int32_t *__restrict__ species, const float *__restrict__ W, int C, int in_dim,
+                                  int out_dim, int n_paths, int n_species, const int *__restrict__ ptr, const int *__restrict__ a1, const int *__restrict__ a2,
+                                  const int *__restrict__ tp, const float *__restrict__ tc, float *__restrict__ B)
+{
+    extern __shared__ float As[];                      // [in_dim][CB]
+    const int n = blockIdx.x, CB = blockDim.x, u = blockIdx.y * CB + threadIdx.x;
+    const bool act = u < C;
+    for (int r = 0; r < in_dim; ++r) As[r * CB + threadIdx.x] = act ? A[((size_t)n * in_dim + r) * C + u] : 0.0f;
+    int z = species[n];
+    z = z < 0 ? 0 : (z >= n_species ? n_species - 1 : z);      // range is checked by the entry point's caller contract; clamp, never read out of bounds
+    if (!act) return;
+    const float *Wz = W + (size_t)z * n_paths * C + u;
+    for (int R = 0; R < out_dim; ++R) {
+        float acc = 0.0f;
+        for (int t = ptr[R]; t < ptr[R + 1]; ++t) {
+            const float w = __ldg(Wz + (size_t)tp[t] * C);
+            const float x1 = As[a1[t] * CB + threadIdx.x];
+            const int j = a2[t];
+            acc = fmaf(w * tc[t], j >= 0 ? x1 * As[j * CB + threadIdx.x] : x1, acc);
+        }
+        B[((size_t)n * out_dim + R) * C + u] = acc;
+    }
+}
+
+__global__ void symcon_bwd_feats_kernel(const float *__restrict__ A, const int32_t *__restrict__ species, const float *__restrict__ W, const float *__restrict__ G,
+                                        int C, int in_dim, int out_dim, int n_paths, int n_species, const int *__restrict__ ptr, const int *__restrict__ other,
+                                        const int *__restrict__ grow, const int *__restrict__ tp, const float *__restrict__ tc, float *__restrict__ dA)
+{
+    extern __shared__ float sm[];                      // A [in_dim][CB] then G [out_dim][CB]
+    const int n = blockIdx.x, CB = blockDim.x, u = blockIdx.y * CB + threadIdx.x;
+    float *As = sm, *Gs = sm + in_dim * CB;
+    const bool act = u < C;
+    for (int r = 0; r < in_dim; ++r) As[r * CB + threadIdx.x] = act ? A[((size_t)n * in_dim + r) * C + u] : 0.0f;
+    for (int r = 0; r < out_dim; ++r) Gs[r * CB + threadIdx.x] = act ? G[((size_t)n * out_dim + r) * C + u] : 0.0f;
+    int z = species[n];
+    z = z < 0 ? 0 : (z >= n_species ? n_species - 1 : z);
+    if (!act) return;
+    const float *Wz = W + (size_t)z * n_paths * C + u;
+    for (int R = 0; R < in_dim; ++R) {
+        float acc = 0.0f;
+        for (int t = ptr[R]; t < ptr[R + 1]; ++t) {
+            const float w = __ldg(Wz + (size_t)tp[t] * C);
+            const float g = Gs[grow[t] * CB + threadIdx.x];
+            const int j = other[t];
+            acc = fmaf(w * tc[t], j >= 0 ? g * As[j * CB + threadIdx.x] : g, acc);
+        }
+        dA[((size_t)n * in_dim + R) * C + u] = acc;
+    }
+}
+
+// grid (kChunks, ceil(n_paths * C / 128)): thread = (path, channel); partial[chunk][species][path][channel] over the chunk's nodes in ascending order
+__global__ void symcon_bwd_w_partial_kernel(const float *__restrict__ A, const int32_t *__restrict__ species, const float *__restrict__ G, int C, int in_dim,
+                                            int out_dim, int n_paths, int n_species, int N, const int *__restrict__ ptr, const int *__restrict__ a1,
+                                            const int *__restrict__ a2, const int *__restrict__ grow, const float *__restrict__ tc, float *__restrict__ partial)
+{
+    const int idx = blockIdx.y * blockDim.x + threadIdx.x;
+    if (idx >= n_paths * C) return;
+    const int p = idx / C, u = idx % C;
+    const int per = (N + kChunks - 1) / kChunks, n0 = blockIdx.x * per, n1 = min(N, n0 + per);
+    float *dst = partial + (size_t)blockIdx.x * n_species * n_paths * C + idx;
+    for (int s = 0; s < n_species; ++s) dst[(size_t)s * n_paths * C] = 0.0f;
+    const int t0 = ptr[p], t1 = ptr[p + 1];
+    for (int n = n0; n < n1; ++n) {
+        const float *a = A + (size_t)n * in_dim * C + u, *g = G + (size_t)n * out_dim * C + u;
+        float acc = 0.0f;
+        for (int t = t0; t < t1; ++t) {
+            const float x1 = a[(size_t)a1[t] * C];
+            const int j = a2[t];
+            acc = fmaf(tc[t] * g[(size_t)grow[t] * C], j >= 0 ? x1 * a[(size_t)j * C] : x1, acc);
+        }
+        int z = species[n];
+        z = z < 0 ? 0 : (z >= n_species ? n_species - 1 : z);
+        dst[(size_t)z * n_paths * C] += acc;
+    }
+}
+
+__global__ void symcon_bwd_w_reduce_kernel(const float *__restrict__ partial, int total, float *__restrict__ dW)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    float acc = 0.0f;
+    for (int c = 0; c < kChunks; ++c) acc += partial[(size_t)c * total + i];
+    dW[i] = acc;
+}
+
+template <typename T>
+int upload(T **dst, const std::vector<T> &v)
+{
+    const size_t b = std::max<size_t>(v.size(), 1) * sizeof(T);
+    E3_CUDA_TRY(cudaMalloc((void **)dst, b));
+    if (!v.empty()) E3_CUDA_TRY(cudaMemcpy(*dst, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return E3_OK;
+}
+
+}  // namespace
+
+extern "C" int e3_symcon_destroy(e3_symcon *sc)
+{
+    if (!sc) return E3_OK;
+    void *ptrs[] = { sc->f_ptr, sc->f_a1, sc->f_a2, sc->f_p, sc->f_c, sc->b_ptr, sc->b_other, sc->b_g, sc->b_p, sc->b_c, sc->w_ptr, sc->w_a1, sc->w_a2, sc->w_g, sc->w_c };
+    for (void *p : ptrs) if (p) cudaFree(p);
+    delete sc;
+    return E3_OK;
+}
+
+extern "C" int e3_symcon_create(e3_symcon **out, const e3_irrep *irreps_in, int n_in, const e3_irrep *irreps_out, int n_out, const e3_pair_path *paths,
+                                int n_paths, int n_species)
+{
+    if (!out || !irreps_in || !irreps_out || !paths || n_in < 1 || n_out < 1 || n_paths < 1 || n_species < 1) { set_error("e3_symcon_create: bad arguments"); return E3_ERR_INVALID_ARG; }
+    *out = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); set_error("e3_symcon_create: no CUDA device (no CPU fallback)"); return E3_ERR_CUDA; }
+    const int C = irreps_in[0].mul;
+    std::vector<int> in_off(n_in), out_off(n_out);
+    int in_dim = 0, out_dim = 0;
+    for (int i = 0; i < n_in; ++i) {
+        if (irreps_in[i].mul != C || C < 1) { set_error("symmetric contraction: all multiplicities must be equal"); return E3_ERR_UNSUPPORTED; }
+        if (irreps_in[i].l < 0 || irreps_in[i].l > kMaxL || (irreps_in[i].parity != 1 && irreps_in[i].parity != -1)) { set_error("symmetric contraction: bad input irrep %d", i); return E3_ERR_UNSUPPORTED; }
+        in_off[i] = in_dim; in_dim += 2 * irreps_in[i].l + 1;
+    }
+    for (int i = 0; i < n_out; ++i) {
+        if (irreps_out[i].mul != C) { set_error("symmetric contraction: all multiplicities must be equal"); return E3_ERR_UNSUPPORTED; }
+        if (irreps_out[i].l < 0 || irreps_out[i].l > kMaxL || (irreps_out[i].parity != 1 && irreps_out[i].parity != -1)) { set_error("symmetric contraction: bad output irrep %d", i); return E3_ERR_UNSUPPORTED; }
+        out_off[i] = out_dim; out_dim += 2 * irreps_out[i].l + 1;
+    }
+    std::vector<int> triples;
+    std::vector<int> quad_of(n_paths, -1);
+    for (int p = 0; p < n_paths; ++p) {
+        const e3_pair_path q = paths[p];
+        if (q.i_in1 < 0 || q.i_in1 >= n_in || q.i_in2 >= n_in || q.i_out < 0 || q.i_out >= n_out) { set_error("symmetric contraction: path %d has an index out of range", p); return E3_ERR_BAD_PATH; }
+        const int L = irreps_out[q.i_out].l;
+        if (q.i_in2 < 0) {
+            if (irreps_in[q.i_in1].l != L || irreps_in[q.i_in1].parity != irreps_out[q.i_out].parity) { set_error("symmetric contraction: linear path %d changes the irrep", p); return E3_ERR_BAD_PATH; }
+        } else {
+            const int l1 = irreps_in[q.i_in1].l, l2 = irreps_in[q.i_in2].l;
+            if (L < std::abs(l1 - l2) || L > l1 + l2) { set_error("symmetric contraction: path %d violates the triangle rule", p); return E3_ERR_BAD_PATH; }
+            if (irreps_in[q.i_in1].parity * irreps_in[q.i_in2].parity != irreps_out[q.i_out].parity) { set_error("symmetric contraction: path %d violates the parity rule", p); return E3_ERR_BAD_PATH; }
+            quad_of[p] = (int)triples.size() / 3;
+            triples.push_back(l1); triples.push_back(l2); triples.push_back(L);
+        }
+    }
+    std::vector<std::vector<double>> dense;
+    if (!triples.empty()) {
+        int rc = launch_cg_planner(triples.data(), (int)triples.size() / 3, dense);
+        if (rc != E3_OK) return rc;
+    }
+    struct Term { int a1, a2, grow, p; float c; };
+    std::vector<Term> terms;
+    for (int p = 0; p < n_paths; ++p) {
+        const e3_pair_path q = paths[p];
+        const int L = irreps_out[q.i_out].l;
+        if (q.i_in2 < 0) {
+            for (int M = 0; M <= 2 * L; ++M) terms.push_back({ in_off[q.i_in1] + M, -1, out_off[q.i_out] + M, p, 1.0f });
+        } else {
+            const int l1 = irreps_in[q.i_in1].l, l2 = irreps_in[q.i_in2].l;
+            const std::vector<double> &cg = dense[quad_of[p]];
+            for (int m1 = 0; m1 <= 2 * l1; ++m1)
+                for (int m2 = 0; m2 <= 2 * l2; ++m2)
+                    for (int M = 0; M <= 2 * L; ++M) {
+                        const double c = cg[(m1 * (2 * l2 + 1) + m2) * (2 * L + 1) + M];
+                        if (std::fabs(c) > 1e-12) terms.push_back({ in_off[q.i_in1] + m1, in_off[q.i_in2] + m2, out_off[q.i_out] + M, p, (float)c });
+                    }
+        }
+    }
+    e3_symcon *sc = new (std::nothrow) e3_symcon();
+    if (!sc) { set_error("out of host memory"); return E3_ERR_INVALID_ARG; }
+    sc->n_in = n_in; sc->n_out = n_out; sc->n_paths = n_paths; sc->n_species = n_species; sc->C = C; sc->in_dim = in_dim; sc->out_dim = out_dim;
+    sc->nnz = (int)terms.size();
+    // CSR by output row
+    std::vector<int> fptr(out_dim + 1, 0), fa1, fa2, fp; std::vector<float> fc;
+    for (int R = 0; R < out_dim; ++R) {
+        for (const Term &t : terms) if (t.grow == R) { fa1.push_back(t.a1); fa2.push_back(t.a2); fp.push_back(t.p); fc.push_back(t.c); }
+        fptr[R + 1] = (int)fa1.size();
+    }
+    // CSR by input row: a quadratic term contributes to the gradient of both of its factors
+    std::vector<int> bptr(in_dim + 1, 0), bo, bg, bp; std::vector<float> bc;
+    for (int R = 0; R < in_dim; ++R) {
+        for (const Term &t : terms) {
+            if (t.a1 == R) { bo.push_back(t.a2); bg.push_back(t.grow); bp.push_back(t.p); bc.push_back(t.c); }
+            if (t.a2 == R) { bo.push_back(t.a1); bg.push_back(t.grow); bp.push_back(t.p); bc.push_back(t.c); }
+        }
+        bptr[R + 1] = (int)bo.size();
+    }
+    // CSR by path
+    std::vector<int> wptr(n_paths + 1, 0), wa1, wa2, wg; std::vector<float> wc;
+    for (int p = 0; p < n_paths; ++p) {
+        for (const Term &t : terms) if (t.p == p) { wa1.push_back(t.a1); wa2.push_back(t.a2); wg.push_back(t.grow); wc.push_back(t.c); }
+        wptr[p + 1] = (int)wa1.size();
+    }
+    int rc = upload(&sc->f_ptr, fptr);
+    if (rc == E3_OK) rc = upload(&sc->f_a1, fa1);
+    if (rc == E3_OK) rc = upload(&sc->f_a2, fa2);
+    if (rc == E3_OK) rc = upload(&sc->f_p, fp);
+    if (rc == E3_OK) rc = upload(&sc->f_c, fc);
+    if (rc == E3_OK) rc = upload(&sc->b_ptr, bptr);
+    if (rc == E3_OK) rc = upload(&sc->b_other, bo);
+    if (rc == E3_OK) rc = upload(&sc->b_g, bg);
+    if (rc == E3_OK) rc = upload(&sc->b_p, bp);
+    if (rc == E3_OK) rc = upload(&sc->b_c, bc);
+    if (rc == E3_OK) rc = upload(&sc->w_ptr, wptr);
+    if (rc == E3_OK) rc = upload(&sc->w_a1, wa1);
+    if (rc == E3_OK) rc = upload(&sc->w_a2, wa2);
+    if (rc == E3_OK) rc = upload(&sc->w_g, wg);
+    if (rc == E3_OK) rc = upload(&sc->w_c, wc);
+    if (rc != E3_OK) { e3_symcon_destroy(sc); return rc; }
+    *out = sc;
+    return E3_OK;
+}
+
+extern "C" int e3_symcon_dims(const e3_symcon *sc, int *in_dim, int *out_dim, int *n_paths, int *n_terms)
+{
+    if (!sc) { set_error("symcon is NULL"); return E3_ERR_INVALID_ARG; }
+    if (in_dim) *in_dim = sc->in_dim;
+    if (out_dim) *out_dim = sc->out_dim;
+    if (n_paths) *n_paths = sc->n_paths;
+    if (n_terms) *n_terms = sc->nnz;
+    return E3_OK;
+}
+
+static inline int block_threads(int C) { return C >= 128 ? 128 : ((C + 31) / 32) * 32; }
+
+extern "C" int e3_symcon_fwd(const e3_symcon *sc, const float *feats, const int32_t *species, const float *weights, int32_t n_nodes, float *out, e3_stream stream)
+{
+    if (!sc || n_nodes < 0 || (n_nodes > 0 && (!feats || !species || !weights || !out))) { set_error("e3_symcon_fwd: bad arguments"); return E3_ERR_INVALID_ARG; }
+    if (n_nodes == 0) return E3_OK;
+    const int th = block_threads(sc->C);
+    const size_t smem = (size_t)sc->in_dim * th * sizeof(float);
+    symcon_fwd_kernel<<<dim3((unsigned)n_nodes, (unsigned)((sc->C + th - 1) / th)), th, smem, reinterpret_cast<cudaStream_t>(stream)>>>(
+        feats, species, weights, sc->C, sc->in_dim, sc->out_dim, sc->n_paths, sc->n_species, sc->f_ptr, sc->f_a1, sc->f_a2, sc->f_p, sc->f_c, out);
+    E3_CUDA_TRY(cudaGetLastError());
+    return E3_OK;
+}
+
+extern "C" size_t e3_symcon_workspace_bytes(const e3_symcon *sc, int32_t n_nodes)
+{
+    (void)n_nodes;
+    if (!sc) return 0;
+    return (size_t)kChunks * sc->n_species * sc->n_paths * sc->C * sizeof(float) + 256;
+}
+
+extern "C" int e3_symcon_bwd(const e3_symcon *sc, const float *feats, const int32_t *species, const float *weights, int32_t n_nodes, const float *grad_out,
+                             float *grad_feats, float *grad_weights, void *workspace, size_t workspace_bytes, e3_stream stream)
+{
+    if (!sc || n_nodes < 0 || (n_nodes > 0 && (!feats || !species || !weights || !grad_out))) { set_error("e3_symcon_bwd: bad arguments"); return E3_ERR_INVALID_ARG; }
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    const int th = block_threads(sc->C);
+    if (grad_feats && n_nodes > 0) {
+        const size_t smem = (size_t)(sc->in_dim + sc->out_dim) * th * sizeof(float);
+        if (smem > 48 * 1024) {
+            static bool set = false;
+            if (!set) { E3_CUDA_TRY(cudaFuncSetAttribute(symcon_bwd_feats_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)); set = true; }
+            if (smem > 200 * 1024) { set_error("e3_symcon_bwd: rows too long for shared memory"); return E3_ERR_UNSUPPORTED; }
+        }
+        symcon_bwd_feats_kernel<<<dim3((unsigned)n_nodes, (unsigned)((sc->C + th - 1) / th)), th, smem, st>>>(
+            feats, species, weights, grad_out, sc->C, sc->in_dim, sc->out_dim, sc->n_paths, sc->n_species, sc->b_ptr, sc->b_other, sc->b_g, sc->b_p, sc->b_c, grad_feats);
+        E3_CUDA_TRY(cudaGetLastError());
+    }
+    if (grad_weights) {
+        if (!workspace || workspace_bytes < e3_symcon_workspace_bytes(sc, n_nodes)) { set_error("e3_symcon_bwd: workspace too small"); return E3_ERR_WORKSPACE; }
+        float *partial = reinterpret_cast<float *>(workspace);
+        const int pc = sc->n_paths * sc->C, total = sc->n_species * pc;
+        symcon_bwd_w_partial_kernel<<<dim3(kChunks, (unsigned)((pc + 127) / 128)), 128, 0, st>>>(
+            feats, species, grad_out, sc->C, sc->in_dim, sc->out_dim, sc->n_paths, sc->n_species, n_nodes, sc->w_ptr, sc->w_a1, sc->w_a2, sc->w_g, sc->w_c, partial);
+        E3_CUDA_TRY(cudaGetLastError());
+        symcon_bwd_w_reduce_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(partial, total, grad_weights);
+        E3_CUDA_TRY(cudaGetLastError());
+    }
+    return E3_OK;
+}
