@@ -381,3 +381,73 @@ def symcon2_bwd(irreps_in, irreps_out, paths, n_species, A, species, W, g):
     if rc:
         raise ValueError(f"oracle symmetric contraction invalid (code {rc})")
     return dA, dW
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# NEXT-4 (the Graph class computes edge vectors from positions and connectivity; L82 "scale model
+# deployment to larger systems"; L298 / L497 cutoff 5 A): neighbour list and receiver-range sharding.  Plain numpy, brute force.
+# The paper prints neither, so both are readings (N1, N2).
+# ------------------------------------------------------------------------------------------------------------------
+def neighbor_build(pos, box, cutoff):
+    """Reading N1.  All pairs, no cell list.  The inclusion test decides an integer (which edges exist), so it is taken in
+    the kernel's precision, IEEE float32 with every operation rounded (no fused multiply-add):
+        d_a = pos[r,a] - pos[s,a];  if box_a > 0:  d_a = d_a - box_a * rint(d_a / box_a)          (minimum image, reading A10)
+        d2  = (d_x*d_x + d_y*d_y) + d_z*d_z;   edge s -> r  iff  s != r and d2 < cutoff*cutoff        (strict, reading A11)
+    box_a = 0 means no periodicity along a; a periodic box_a must be >= 2*cutoff (one image at most).  Edges are ordered by
+    receiver, ties by ascending sender (A11).  Returns senders, receivers (int32), vec [E,3] float32 (= d) and row_ptr.
+    Pins (tests/test_oracle_nb.py): scipy's cKDTree on the same positions, the simple cubic lattice's coordination numbers,
+    pair symmetry, python-loop brute force on an open cluster, the harness graph of config 1."""
+    pos = np.ascontiguousarray(pos, dtype=np.float32)
+    box = np.asarray(box, dtype=np.float32).reshape(3)
+    rc = np.float32(cutoff)
+    if any(b > 0 and b < 2 * rc for b in box):
+        raise ValueError("a periodic box edge must be at least twice the cutoff")
+    rc2 = rc * rc
+    n = pos.shape[0]
+    snd, rcv, vec = [], [], []
+    for r0 in range(0, n, 256):                                   # receivers in slabs only to bound memory
+        pr = pos[r0:r0 + 256]
+        d = pr[:, None, :] - pos[None, :, :]                       # [R, N, 3] float32
+        for a in range(3):
+            if box[a] > 0:
+                d[:, :, a] = d[:, :, a] - box[a] * np.rint(d[:, :, a] / box[a])
+        d2 = (d[:, :, 0] * d[:, :, 0] + d[:, :, 1] * d[:, :, 1]) + d[:, :, 2] * d[:, :, 2]
+        keep = d2 < rc2
+        keep[np.arange(pr.shape[0]), np.arange(r0, r0 + pr.shape[0])] = False
+        rr, ss = np.nonzero(keep)                                  # row-major: receiver ascending, then sender ascending
+        rcv.append(rr + r0); snd.append(ss); vec.append(d[rr, ss])
+    snd = np.concatenate(snd).astype(np.int32) if snd else np.zeros(0, np.int32)
+    rcv = np.concatenate(rcv).astype(np.int32) if rcv else np.zeros(0, np.int32)
+    vec = np.concatenate(vec).astype(np.float32) if vec else np.zeros((0, 3), np.float32)
+    row_ptr = np.zeros(n + 1, np.int32)
+    np.add.at(row_ptr, rcv + 1, 1)
+    return snd, rcv, vec, np.cumsum(row_ptr).astype(np.int32)
+
+
+def shard_ranges(receivers, n_nodes, world):
+    """Reading N2: contiguous receiver ranges of about equal EDGE counts.  Boundary k (1 <= k < world) is the
+    receiver of edge floor(k*E/world) (n_nodes when that index is E); boundaries are made non-decreasing; rank k owns the atoms
+    [b_k, b_{k+1}) and all their in-edges."""
+    receivers = np.asarray(receivers)
+    E = receivers.shape[0]
+    b = [0]
+    for k in range(1, world):
+        t = (k * E) // world
+        b.append(max(b[-1], int(receivers[t]) if t < E else n_nodes))
+    b.append(n_nodes)
+    return b
+
+
+def shard_local_graph(senders, receivers, n_nodes, world, rank):
+    """Reading N2: the local problem of one rank.  Local node ids: the owned atoms b_k..b_{k+1}-1 first (in order), then the halo
+    = the senders of the rank's edges that it does not own, ascending.  Returns dict(lo, hi, e_lo, e_hi, halo (global ids),
+    senders_local, receivers_local)."""
+    senders, receivers = np.asarray(senders), np.asarray(receivers)
+    b = shard_ranges(receivers, n_nodes, world)
+    lo, hi = b[rank], b[rank + 1]
+    e_lo, e_hi = int(np.searchsorted(receivers, lo, "left")), int(np.searchsorted(receivers, hi, "left"))
+    s, r = senders[e_lo:e_hi], receivers[e_lo:e_hi]
+    halo = np.unique(s[(s < lo) | (s >= hi)])
+    s_loc = np.where((s >= lo) & (s < hi), s - lo, (hi - lo) + np.searchsorted(halo, s))
+    return dict(lo=lo, hi=hi, e_lo=e_lo, e_hi=e_hi, halo=halo.astype(np.int32), senders_local=s_loc.astype(np.int32),
+                receivers_local=(r - lo).astype(np.int32))
