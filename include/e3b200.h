@@ -50,7 +50,7 @@ enum {
     E3_OK = 0,
     E3_ERR_INVALID_ARG = 1,   /* null pointer, negative size, index out of range                     */
     E3_ERR_BAD_PATH = 2,      /* triangle rule, parity rule or irrep index violated                  */
-    E3_ERR_UNSUPPORTED = 3,   /* l > 3, unequal multiplicities, C*dtype row not 4-byte aligned, ...  */
+    E3_ERR_UNSUPPORTED = 3,   /* l > 3, unequal multiplicities not multiples of 4, odd row alignment */
     E3_ERR_UNSORTED = 4,      /* receivers not ascending (only when validation was requested)        */
     E3_ERR_CUDA = 5,          /* CUDA runtime error or no device                                     */
     E3_ERR_JIT = 6,           /* run-time specialisation (NVRTC) of the plan's kernels failed        */
@@ -75,7 +75,13 @@ int e3_all_paths(const e3_irrep *irreps_in, int n_in, int sh_lmax, int out_lmax,
  * change, reading A4), compacts them to sparse (m1,m2,m3,coef) lists and specialises the
  * forward and VJP kernels for this plan (coefficients become FFMA immediates).  Needs a device;
  * synchronises; takes O(seconds) once.  A path whose i_out is shared with another path ADDS
- * into that block (A6).  Limits: l <= 3 everywhere, all multiplicities equal.
+ * into that block (A6).  Limits: l <= 3 everywhere.
+ * Multiplicities (NEXT-4, NequIP's `64x0e + 64x0o + 32x1o + 32x1e + 32x2e + 32x2o`): when all
+ * irreps have the same multiplicity C the layouts are those of A7/A8.  Otherwise every multiplicity must be a multiple of 4, a
+ * path's input and output irrep must have the same multiplicity (a channelwise path keeps it; E3_ERR_BAD_PATH otherwise), and
+ * the layouts are: node row = irrep blocks back to back, block i = (2l_i+1) x mul_i values at index m*mul_i + u; weights row =
+ * mul(path) values per path, paths back to back (e3_plan_sizes returns the three row lengths).  Such a plan runs one generated
+ * kernel pair per multiplicity class over the same rows; every entry point below accepts it.
  * Environment: E3_TUNE="key=value,..." overrides launch-shape heuristics (never results);
  * E3_JIT_CACHE=0 disables the compiled-kernel cache (speed only).  The cache lives in a per-user directory of mode 0700
  * ($E3_JIT_DIR, else $XDG_CACHE_HOME/e3b200_jit, else /tmp/e3b200_jit_<uid>; refused if not owned by the caller or
@@ -88,6 +94,9 @@ int e3_plan_destroy(e3_plan *plan);
 /* in_dim = sum(2l+1) over irreps_in, sh_dim = (sh_lmax+1)^2, out_dim likewise over irreps_out,
  * weights_per_edge = n_paths * C, nnz_total = number of non-zero real CG coefficients. */
 int e3_plan_dims(const e3_plan *plan, int *in_dim, int *sh_dim, int *out_dim, int *weights_per_edge, int *nnz_total);
+/* Row lengths in ELEMENTS: feats / grad_feats rows (sum (2l+1)*mul over irreps_in), out / grad_out rows (likewise over irreps_out)
+ * and weights / grad_weights rows (sum of mul over paths).  Any pointer may be NULL. */
+int e3_plan_sizes(const e3_plan *plan, int64_t *feats_per_node, int64_t *out_per_node, int64_t *weights_per_edge);
 /* Host copy of path `path`'s sparse CG list (m indices are 0-based: m_true + l).  Pass m1 == NULL
  * to query *nnz only.  Order: m1, then m2, then m3 ascending. */
 int e3_plan_get_cg(const e3_plan *plan, int path, int *m1, int *m2, int *m3, double *coef, int *nnz);

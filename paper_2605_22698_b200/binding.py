@@ -20,7 +20,7 @@ E3_OK, E3_ERR_INVALID_ARG, E3_ERR_BAD_PATH, E3_ERR_UNSUPPORTED, E3_ERR_UNSORTED,
 
 SYMBOLS = [
     "e3_status_string", "e3_last_error", "e3_all_paths", "e3_plan_create", "e3_plan_destroy", "e3_plan_dims",
-    "e3_plan_get_cg", "e3_plan_kernel_info", "e3_plan_work", "e3_jit_check", "e3_graph_workspace_bytes",
+    "e3_plan_sizes", "e3_plan_get_cg", "e3_plan_kernel_info", "e3_plan_work", "e3_jit_check", "e3_graph_workspace_bytes",
     "e3_graph_prepare", "e3_sh_fwd", "e3_sh_bwd", "e3_tp_scatter_fwd", "e3_bwd_workspace_bytes", "e3_tp_scatter_bwd",
     "e3_force_reduce", "e3_profile_set_mid_event", "e3_measure_fp32_peak", "e3_session_create", "e3_session_destroy", "e3_session_run_host",
     "e3_vjp_vjp_workspace_bytes", "e3_tp_scatter_vjp_vjp", "e3_sh_bwd_bwd",
@@ -122,7 +122,10 @@ class Plan:
         vals = [C.c_int() for _ in range(5)]
         _check(lib().e3_plan_dims(handle, *[C.byref(v) for v in vals]), "e3_plan_dims")
         self.in_dim, self.sh_dim, self.out_dim, self.weights_per_edge, self.nnz_total = [v.value for v in vals]
-        self.channels = int(irreps_in[0][2])
+        self.channels = int(irreps_in[0][2])      # of the first irrep; rows are sized by the three fields below
+        sz = [C.c_int64() for _ in range(3)]
+        _check(lib().e3_plan_sizes(handle, *[C.byref(v) for v in sz]), "e3_plan_sizes")
+        self.feats_per_node, self.out_per_node, self.weights_per_edge = [int(v.value) for v in sz]
         self.n_paths = len(paths)
         self.storage = torch.bfloat16 if dtype == E3_BF16 else torch.float32
 
@@ -214,7 +217,7 @@ def e3_tp_scatter_fwd(plan: Plan, feats, sh, weights, senders, receivers, row_pt
     _dev(senders, torch.int32); _dev(row_ptr, torch.int32)
     E = senders.numel()
     if out is None:
-        out = torch.empty((n_nodes, plan.out_dim * plan.channels), dtype=torch.float32, device=feats.device)
+        out = torch.empty((n_nodes, plan.out_per_node), dtype=torch.float32, device=feats.device)
     _check(lib().e3_tp_scatter_fwd(plan.handle, _ptr(feats), _ptr(sh), _ptr(weights), _ptr(senders), _ptr(receivers),
                                    _ptr(row_ptr), C.c_int64(E), C.c_int32(n_nodes), _ptr(_dev(out, torch.float32)),
                                    _stream(stream)), "e3_tp_scatter_fwd")
@@ -238,7 +241,7 @@ def e3_tp_scatter_bwd(plan: Plan, feats, sh, weights, senders, receivers, row_pt
     E = senders.numel()
     dev = feats.device
     if grad_feats is None:
-        grad_feats = torch.empty((n_nodes, plan.in_dim * plan.channels), dtype=torch.float32, device=dev)
+        grad_feats = torch.empty((n_nodes, plan.feats_per_node), dtype=torch.float32, device=dev)
     if grad_sh is None:
         grad_sh = torch.empty((E, plan.sh_dim), dtype=torch.float32, device=dev)
     if grad_weights is None and want_grad_weights:
@@ -350,7 +353,7 @@ def e3_tp_scatter_vjp_vjp(plan: Plan, feats, sh, weights, senders, receivers, ro
     E = senders.numel()
     dev = feats.device
     f32 = torch.float32
-    outs = {"gg": (n_nodes, plan.out_dim * plan.channels), "gx": (n_nodes, plan.in_dim * plan.channels),
+    outs = {"gg": (n_nodes, plan.out_per_node), "gx": (n_nodes, plan.feats_per_node),
             "gY": (E, plan.sh_dim), "gw": (E, plan.weights_per_edge)}
     bufs = {k: (torch.empty(shape, dtype=f32, device=dev) if k in want else None) for k, shape in outs.items()}
     nbytes = int(lib().e3_vjp_vjp_workspace_bytes(plan.handle, C.c_int64(E), C.c_int32(n_nodes)))

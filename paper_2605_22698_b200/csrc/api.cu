@@ -61,21 +61,10 @@ static int plan_generate(e3_plan &pl, const char *src_path)
     return jit_compile(pl.bwd, f2);
 }
 
-extern "C" int e3_plan_create(e3_plan **plan, const e3_irrep *irreps_in, int n_in, int sh_lmax, const e3_irrep *irreps_out,
-                              int n_out, const e3_path *paths, int n_paths, e3_dtype dtype)
+// generate + compile + load the two kernels of a regular plan (or of one sub-plan of a composite)
+static int plan_finish(e3_plan *pl)
 {
-    if (!plan) { set_error("e3_plan_create: plan is NULL"); return E3_ERR_INVALID_ARG; }
-    *plan = nullptr;
-    int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
-        cudaGetLastError();
-        set_error("e3_plan_create: no CUDA device (this library has no CPU fallback)");
-        return E3_ERR_CUDA;
-    }
-    e3_plan *pl = new (std::nothrow) e3_plan();
-    if (!pl) { set_error("out of host memory"); return E3_ERR_INVALID_ARG; }
-    int rc = plan_build_tables(*pl, irreps_in, n_in, sh_lmax, irreps_out, n_out, paths, n_paths, dtype, /*cg_on_device=*/true);
-    if (rc == E3_OK) rc = plan_generate(*pl, nullptr);
+    int rc = plan_generate(*pl, nullptr);
     if (rc == E3_OK) rc = jit_load(pl->fwd);
     if (rc == E3_OK) rc = jit_load(pl->bwd);
     const int fwd_smem_max = (rc == E3_OK && pl->fwd_v3) ? v3_smem(pl, v3_fsplit_max(pl)) : pl->fwd.smem_dyn;
@@ -99,18 +88,58 @@ extern "C" int e3_plan_create(e3_plan **plan, const e3_irrep *irreps_in, int n_i
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, (const void *)pl->bwd.fn, pl->bwd.threads, pl->bwd.smem_dyn) == cudaSuccess && b > 0) pl->bwd_ctas_per_sm = b;
         cudaGetLastError();
     }
-    if (rc != E3_OK) { jit_unload(pl->fwd); jit_unload(pl->bwd); if (pl->zeros) cudaFree(pl->zeros); delete pl; return rc; }
+    return rc;
+}
+
+static void plan_free(e3_plan *pl)
+{
+    if (!pl) return;
+    for (e3_plan *sp : pl->subs) plan_free(sp);
+    jit_unload(pl->fwd);
+    jit_unload(pl->bwd);
+    if (pl->zeros) cudaFree(pl->zeros);
+    delete pl;
+}
+
+extern "C" int e3_plan_create(e3_plan **plan, const e3_irrep *irreps_in, int n_in, int sh_lmax, const e3_irrep *irreps_out,
+                              int n_out, const e3_path *paths, int n_paths, e3_dtype dtype)
+{
+    if (!plan) { set_error("e3_plan_create: plan is NULL"); return E3_ERR_INVALID_ARG; }
+    *plan = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        set_error("e3_plan_create: no CUDA device (this library has no CPU fallback)");
+        return E3_ERR_CUDA;
+    }
+    e3_plan *pl = new (std::nothrow) e3_plan();
+    if (!pl) { set_error("out of host memory"); return E3_ERR_INVALID_ARG; }
+    int rc;
+    if (plan_is_composite(irreps_in, n_in, irreps_out, n_out)) {
+        // NEXT-4: per-irrep multiplicities -> one generated sub-plan per multiplicity class
+        rc = plan_build_composite(*pl, irreps_in, n_in, sh_lmax, irreps_out, n_out, paths, n_paths, dtype, /*cg_on_device=*/true);
+        for (size_t k = 0; rc == E3_OK && k < pl->subs.size(); ++k) rc = plan_finish(pl->subs[k]);
+    } else {
+        rc = plan_build_tables(*pl, irreps_in, n_in, sh_lmax, irreps_out, n_out, paths, n_paths, dtype, /*cg_on_device=*/true);
+        if (rc == E3_OK) rc = plan_finish(pl);
+    }
+    if (rc != E3_OK) { plan_free(pl); return rc; }
     *plan = pl;
     return E3_OK;
 }
 
 extern "C" int e3_plan_destroy(e3_plan *plan)
 {
-    if (!plan) return E3_OK;
-    jit_unload(plan->fwd);
-    jit_unload(plan->bwd);
-    if (plan->zeros) cudaFree(plan->zeros);
-    delete plan;
+    plan_free(plan);
+    return E3_OK;
+}
+
+extern "C" int e3_plan_sizes(const e3_plan *plan, int64_t *feats_per_node, int64_t *out_per_node, int64_t *weights_per_edge)
+{
+    if (!plan) { set_error("plan is NULL"); return E3_ERR_INVALID_ARG; }
+    if (feats_per_node) *feats_per_node = plan->in_size();
+    if (out_per_node) *out_per_node = plan->out_size();
+    if (weights_per_edge) *weights_per_edge = plan->w_size();
     return E3_OK;
 }
 
@@ -120,7 +149,7 @@ extern "C" int e3_plan_dims(const e3_plan *plan, int *in_dim, int *sh_dim, int *
     if (in_dim) *in_dim = plan->in_dim;
     if (sh_dim) *sh_dim = plan->sh_dim;
     if (out_dim) *out_dim = plan->out_dim;
-    if (weights_per_edge) *weights_per_edge = (int)plan->paths.size() * plan->C;
+    if (weights_per_edge) *weights_per_edge = plan->w_size();
     if (nnz_total) *nnz_total = plan->nnz_total;
     return E3_OK;
 }
@@ -128,6 +157,7 @@ extern "C" int e3_plan_dims(const e3_plan *plan, int *in_dim, int *sh_dim, int *
 extern "C" int e3_plan_get_cg(const e3_plan *plan, int path, int *m1, int *m2, int *m3, double *coef, int *nnz)
 {
     if (!plan || !nnz || path < 0 || path >= (int)plan->paths.size()) { set_error("e3_plan_get_cg: bad arguments"); return E3_ERR_INVALID_ARG; }
+    if (!plan->subs.empty()) return e3_plan_get_cg(plan->subs[plan->path_map[path].first], plan->path_map[path].second, m1, m2, m3, coef, nnz);
     const PathInfo &pi = plan->paths[path];
     *nnz = (int)pi.nz.size();
     if (m1 && m2 && m3 && coef)
@@ -139,6 +169,21 @@ extern "C" int e3_plan_kernel_info(const e3_plan *plan, int which, int *regs, in
                                    int *threads_per_block, int *n_roles, int *channels_per_lane)
 {
     if (!plan || (which != 0 && which != 1)) { set_error("e3_plan_kernel_info: bad arguments"); return E3_ERR_INVALID_ARG; }
+    if (!plan->subs.empty()) {
+        int a[6] = { 0, 0, 0, 0, 0, 0 };
+        for (const e3_plan *sp : plan->subs) {
+            int b[6];
+            e3_plan_kernel_info(sp, which, &b[0], &b[1], &b[2], &b[3], &b[4], &b[5]);
+            for (int i = 0; i < 6; ++i) a[i] = i == 4 ? a[i] + b[i] : std::max(a[i], b[i]);
+        }
+        if (regs) *regs = a[0];
+        if (spill_bytes) *spill_bytes = a[1];
+        if (smem_bytes) *smem_bytes = a[2];
+        if (threads_per_block) *threads_per_block = a[3];
+        if (n_roles) *n_roles = a[4];
+        if (channels_per_lane) *channels_per_lane = a[5];
+        return E3_OK;
+    }
     const JitKernel &k = which == 0 ? plan->fwd : plan->bwd;
     if (regs) *regs = k.regs;
     if (spill_bytes) *spill_bytes = k.spill;
@@ -153,6 +198,12 @@ extern "C" int e3_plan_work(const e3_plan *plan, double *fwd_flop_per_edge, doub
 {
     if (!plan) { set_error("plan is NULL"); return E3_ERR_INVALID_ARG; }
     double f = 0, b = 0;
+    for (const e3_plan *sp : plan->subs) {
+        double f1 = 0, b1 = 0;
+        e3_plan_work(sp, &f1, &b1);
+        f += f1; b += b1;
+    }
+    if (plan->subs.empty())
     for (const PathInfo &pi : plan->paths) {
         f += plan->C * (2.0 * pi.nzM + 2.0 * (2 * pi.l3 + 1)) + 2.0 * pi.nz.size();
         b += plan->C * (6.0 * pi.nzM + 3.0 * (2 * pi.l3 + 1)) + 4.0 * pi.nz.size();
@@ -167,6 +218,24 @@ extern "C" int e3_jit_check(const e3_irrep *irreps_in, int n_in, int sh_lmax, co
                             int *fwd_spill, int *bwd_regs, int *bwd_spill)
 {
     e3_plan pl;
+    if (plan_is_composite(irreps_in, n_in, irreps_out, n_out)) {
+        int rc = plan_build_composite(pl, irreps_in, n_in, sh_lmax, irreps_out, n_out, paths, n_paths, dtype, /*cg_on_device=*/false);
+        int v[4] = { 0, 0, 0, 0 };
+        for (size_t k = 0; rc == E3_OK && k < pl.subs.size(); ++k) {
+            const std::string sp = src_path ? std::string(src_path) + ".class" + std::to_string(k) : std::string();
+            rc = plan_generate(*pl.subs[k], src_path ? sp.c_str() : nullptr);
+            v[0] = std::max(v[0], pl.subs[k]->fwd.regs); v[1] = std::max(v[1], pl.subs[k]->fwd.spill);
+            v[2] = std::max(v[2], pl.subs[k]->bwd.regs); v[3] = std::max(v[3], pl.subs[k]->bwd.spill);
+        }
+        for (e3_plan *sp : pl.subs) delete sp;
+        pl.subs.clear();
+        if (rc != E3_OK) return rc;
+        if (fwd_regs) *fwd_regs = v[0];
+        if (fwd_spill) *fwd_spill = v[1];
+        if (bwd_regs) *bwd_regs = v[2];
+        if (bwd_spill) *bwd_spill = v[3];
+        return E3_OK;
+    }
     int rc = plan_build_tables(pl, irreps_in, n_in, sh_lmax, irreps_out, n_out, paths, n_paths, dtype, /*cg_on_device=*/false);
     if (rc == E3_OK) rc = plan_generate(pl, src_path);
     if (rc != E3_OK) return rc;
@@ -229,6 +298,13 @@ static int launch_fwd(const e3_plan *plan, const void *feats, const void *sh, co
 {
     if (heur_nodes < 0) heur_nodes = n_nodes;     // launch-shape heuristics follow the size of the WHOLE graph
     if (n_nodes == 0) return E3_OK;
+    if (!plan->subs.empty()) {                    // composite: every multiplicity class writes its own output blocks
+        for (const e3_plan *sp : plan->subs) {
+            const int rc = launch_fwd(sp, feats, sh, weights, senders, row_ptr, n_nodes, out, st, heur_nodes);
+            if (rc != E3_OK) return rc;
+        }
+        return E3_OK;
+    }
     if (!plan->fwd.fn) { set_error("plan has no loaded forward kernel"); return E3_ERR_CUDA; }
     // small graphs (v2 kernels): `fsplit` warps share one (receiver, role) so that the grid covers the machine
     // several times over; the result depends on fsplit only through the (fixed) summation grouping
@@ -293,28 +369,49 @@ extern "C" int e3_tp_scatter_fwd(const e3_plan *plan, const void *feats, const v
     return launch_fwd(plan, feats, sh, weights, senders, row_ptr, n_nodes, out, S(stream));
 }
 
+// partial grad_sh buffers of the VJP: one per backward role, for a composite one per (class, role); 0 = written in place
+static int gsh_parts(const e3_plan *plan)
+{
+    if (!plan->subs.empty()) {
+        int n = 0;
+        for (const e3_plan *sp : plan->subs) n += sp->bwd_v2 ? sp->bwd_nroles : 1;
+        return n;
+    }
+    return (plan->bwd_v2 && plan->bwd_nroles > 1) ? plan->bwd_nroles : 0;
+}
+
 extern "C" size_t e3_bwd_workspace_bytes(const e3_plan *plan, int64_t n_edges, int32_t n_nodes)
 {
     (void)n_nodes;
     if (!plan || n_edges < 0) return 0;
-    size_t b = (((size_t)n_edges * plan->in_dim * plan->C * sizeof(float) + 255) / 256) * 256 + 256;     // per-edge grad_feats rows
-    if (plan->bwd_v2 && plan->bwd_nroles > 1) b += (size_t)plan->bwd_nroles * n_edges * plan->sh_dim * sizeof(float) + 256;   // per-role grad_sh
+    size_t b = (((size_t)n_edges * plan->in_size() * sizeof(float) + 255) / 256) * 256 + 256;     // per-edge grad_feats rows
+    b += (size_t)gsh_parts(plan) * n_edges * plan->sh_dim * sizeof(float) + 256;   // per-role (and per-class) grad_sh
     return b;
 }
 
 static size_t gsh_parts_offset(const e3_plan *plan, int64_t n_edges)
 {
-    return (((size_t)n_edges * plan->in_dim * plan->C * sizeof(float) + 255) / 256) * 256;
+    return (((size_t)n_edges * plan->in_size() * sizeof(float) + 255) / 256) * 256;
 }
 
 // first VJP phase for a receiver range (offset row_ptr / grad_out pointers, absolute edge- and sender-indexed tensors):
 // grad_weights, per-edge grad_feats rows (workspace) and grad_sh (per-role partial buffers when the plan has several roles)
 static int launch_bwd_phase1(const e3_plan *plan, const void *feats, const void *sh, const void *weights, const int32_t *senders,
                              const int32_t *row_ptr, int32_t n_nodes, const float *grad_out, float *grad_sh, void *grad_weights,
-                             void *workspace, int64_t n_edges_total, cudaStream_t st, int32_t heur_nodes = -1)
+                             void *workspace, int64_t n_edges_total, cudaStream_t st, int32_t heur_nodes = -1, float *gsh_part = nullptr)
 {
     if (n_nodes == 0 || n_edges_total == 0) return E3_OK;
     if (heur_nodes < 1) heur_nodes = n_nodes;
+    if (!plan->subs.empty()) {       // composite: the classes share the per-edge workspace rows; each (class, role) has its grad_sh part
+        float *parts = reinterpret_cast<float *>(reinterpret_cast<char *>(workspace) + gsh_parts_offset(plan, n_edges_total));
+        for (const e3_plan *sp : plan->subs) {
+            const int rc = launch_bwd_phase1(sp, feats, sh, weights, senders, row_ptr, n_nodes, grad_out, grad_sh, grad_weights, workspace,
+                                             n_edges_total, st, heur_nodes, parts);
+            if (rc != E3_OK) return rc;
+            parts += (size_t)(sp->bwd_v2 ? sp->bwd_nroles : 1) * n_edges_total * plan->sh_dim;
+        }
+        return E3_OK;
+    }
     if (!plan->bwd.fn) { set_error("plan has no loaded backward kernel"); return E3_ERR_CUDA; }
     float *dxe = (float *)workspace;
     const int roles = plan->bwd_v2 ? plan->bwd_nroles : 1;
@@ -335,7 +432,8 @@ static int launch_bwd_phase1(const e3_plan *plan, const void *feats, const void 
         grid = chunks * plan->bwd_chunk * plan->bwd_nroles * split;
     }
     if (grid > 0x7fffffffLL) { set_error("grid too large"); return E3_ERR_UNSUPPORTED; }
-    float *gsh_arg = roles > 1 ? reinterpret_cast<float *>(reinterpret_cast<char *>(workspace) + gsh_parts_offset(plan, n_edges_total)) : grad_sh;
+    float *gsh_arg = gsh_part ? gsh_part
+                              : (roles > 1 ? reinterpret_cast<float *>(reinterpret_cast<char *>(workspace) + gsh_parts_offset(plan, n_edges_total)) : grad_sh);
     long long ne = n_edges_total;
     void *args[] = { (void *)&feats, (void *)&sh, (void *)&weights, (void *)&senders, (void *)&row_ptr, (void *)&grad_out,
                      (void *)&dxe, (void *)&gsh_arg, (void *)&grad_weights, (void *)&n_nodes, (void *)&split, (void *)&ne };
@@ -347,9 +445,9 @@ static int launch_bwd_phase1(const e3_plan *plan, const void *feats, const void 
 static int launch_bwd_phase2(const e3_plan *plan, const int32_t *perm_s, const int32_t *col_ptr, int64_t n_edges, int32_t n_nodes,
                              float *grad_feats, float *grad_sh, void *workspace, cudaStream_t st)
 {
-    const int roles = plan->bwd_v2 ? plan->bwd_nroles : 1;
-    int rc = launch_dx_reduce((const float *)workspace, perm_s, col_ptr, n_nodes, plan->in_dim * plan->C, grad_feats, st);
-    if (rc == E3_OK && roles > 1 && n_edges > 0)
+    const int roles = gsh_parts(plan);
+    int rc = launch_dx_reduce((const float *)workspace, perm_s, col_ptr, n_nodes, plan->in_size(), grad_feats, st);
+    if (rc == E3_OK && roles > 0 && n_edges > 0)
         rc = launch_gsh_reduce(reinterpret_cast<const float *>(reinterpret_cast<const char *>(workspace) + gsh_parts_offset(plan, n_edges)),
                                roles, n_edges * plan->sh_dim, grad_sh, st);
     return rc;
@@ -395,9 +493,8 @@ extern "C" size_t e3_vjp_vjp_workspace_bytes(const e3_plan *plan, int64_t n_edge
 {
     if (!plan || n_edges < 0 || n_nodes < 0) return 0;
     auto up = [](size_t b) { return ((b + 255) / 256) * 256; };
-    const size_t C = plan->C;
-    return up(e3_bwd_workspace_bytes(plan, n_edges, n_nodes)) + up((size_t)n_nodes * plan->out_dim * C * 4) + up((size_t)n_nodes * plan->in_dim * C * 4) +
-           up((size_t)n_edges * plan->sh_dim * 4) + up((size_t)n_edges * plan->paths.size() * C * 4) + 256;
+    return up(e3_bwd_workspace_bytes(plan, n_edges, n_nodes)) + up((size_t)n_nodes * plan->out_size() * 4) + up((size_t)n_nodes * plan->in_size() * 4) +
+           up((size_t)n_edges * plan->sh_dim * 4) + up((size_t)n_edges * plan->w_size() * 4) + 256;
 }
 
 extern "C" int e3_tp_scatter_vjp_vjp(const e3_plan *plan, const void *feats, const void *sh, const void *weights, const int32_t *senders,
@@ -421,8 +518,8 @@ extern "C" int e3_tp_scatter_vjp_vjp(const e3_plan *plan, const void *feats, con
     if (n_nodes == 0) return E3_OK;
     cudaStream_t st = S(stream);
     auto up = [](size_t b) { return ((b + 255) / 256) * 256; };
-    const size_t C = plan->C, n_out = (size_t)n_nodes * plan->out_dim * C, n_in = (size_t)n_nodes * plan->in_dim * C;
-    const size_t n_sh = (size_t)n_edges * plan->sh_dim, n_w = (size_t)n_edges * plan->paths.size() * C;
+    const size_t n_out = (size_t)n_nodes * plan->out_size(), n_in = (size_t)n_nodes * plan->in_size();
+    const size_t n_sh = (size_t)n_edges * plan->sh_dim, n_w = (size_t)n_edges * plan->w_size();
     char *wp = (char *)workspace;
     void *bws = wp; wp += up(e3_bwd_workspace_bytes(plan, n_edges, n_nodes));
     float *t_out = (float *)wp; wp += up(n_out * 4);
@@ -547,7 +644,7 @@ extern "C" int e3_session_create(e3_session **session, const e3_plan *plan, int6
     if (!s) { set_error("out of host memory"); return E3_ERR_INVALID_ARG; }
     s->plan = plan; s->max_edges = max_edges; s->max_nodes = max_nodes;
     const size_t E = (size_t)max_edges + 1, N = (size_t)max_nodes + 1, es = esize(plan);
-    const size_t P = plan->paths.size(), C = plan->C;
+    const size_t in_row = (size_t)plan->in_size(), out_row = (size_t)plan->out_size(), w_row = (size_t)plan->w_size();
     s->ws_bytes = e3_bwd_workspace_bytes(plan, max_edges, max_nodes);
     s->gws_bytes = graph_workspace_bytes(max_edges, max_nodes);
     cudaError_t e = cudaStreamCreateWithFlags(&s->stream, cudaStreamNonBlocking);
@@ -562,10 +659,10 @@ extern "C" int e3_session_create(e3_session **session, const e3_plan *plan, int6
     }
 #define SALLOC(ptr, bytes) if (e == cudaSuccess) e = cudaMalloc((void **)&(ptr), (bytes))
     SALLOC(s->vec, E * 3 * 4); SALLOC(s->gvec, E * 3 * 4); SALLOC(s->forces, N * 3 * 4);
-    SALLOC(s->feats, N * plan->in_dim * C * es); SALLOC(s->gfeats, N * plan->in_dim * C * 4);
-    SALLOC(s->out, N * plan->out_dim * C * 4); SALLOC(s->gout, N * plan->out_dim * C * 4);
+    SALLOC(s->feats, N * in_row * es); SALLOC(s->gfeats, N * in_row * 4);
+    SALLOC(s->out, N * out_row * 4); SALLOC(s->gout, N * out_row * 4);
     SALLOC(s->sh, E * plan->sh_dim * es); SALLOC(s->gsh, E * plan->sh_dim * 4);
-    SALLOC(s->weights, E * P * C * es); SALLOC(s->gweights, E * P * C * es);
+    SALLOC(s->weights, E * w_row * es); SALLOC(s->gweights, E * w_row * es);
     SALLOC(s->ws, s->ws_bytes); SALLOC(s->gws, s->gws_bytes);
     SALLOC(s->snd, E * 4); SALLOC(s->rcv, E * 4); SALLOC(s->row_ptr, (N + 1) * 4); SALLOC(s->perm_s, E * 4); SALLOC(s->col_ptr, (N + 1) * 4);
 #undef SALLOC
@@ -603,8 +700,8 @@ static int session_run_host_impl(e3_session *s, const float *vec_h, const void *
         }
     }
     const e3_plan *pl = s->plan;
-    const size_t E = (size_t)n_edges, N = (size_t)n_nodes, es = esize(pl), P = pl->paths.size(), C = pl->C;
-    const size_t in_row = (size_t)pl->in_dim * C, out_row = (size_t)pl->out_dim * C, w_row = P * C;
+    const size_t E = (size_t)n_edges, N = (size_t)n_nodes, es = esize(pl);
+    const size_t in_row = (size_t)pl->in_size(), out_row = (size_t)pl->out_size(), w_row = (size_t)pl->w_size();
     cudaStream_t st = s->stream, sin = s->stream_in, sout = s->stream_out;
     int64_t up = 0, down = 0;
 #define H2D(stream_, dst, src, bytes) do { if ((bytes) > 0) { E3_CUDA_TRY(cudaMemcpyAsync((dst), (src), (bytes), cudaMemcpyHostToDevice, (stream_))); up += (int64_t)(bytes); } } while (0)

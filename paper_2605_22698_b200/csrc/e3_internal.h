@@ -102,6 +102,36 @@ struct e3_plan {
     int n_sm = 148;            // SM count of the device the plan was created on
     e3::JitKernel fwd, bwd;
     cudaEvent_t mid_event = nullptr;   // profiling aid, see e3_profile_set_mid_event
+
+    // Element layout of a node row / a weights row.  A regular plan (all multiplicities equal to C) has its irrep blocks back to
+    // back, (2l+1)*C elements each.  NEXT-4, unequal multiplicities: the plan is a COMPOSITE of one sub-plan per multiplicity
+    // class (`subs`, each a regular generated plan over the irreps and paths of that class) whose kernels address the rows of the
+    // whole plan: strides and block offsets are overridden by the vectors below (empty = regular layout).
+    std::vector<e3_plan *> subs;                 // composite: one sub-plan per multiplicity class (owned)
+    std::vector<std::pair<int, int>> path_map;   // composite: path p of the caller = path .second of subs[.first]
+    int in_size_all = 0, out_size_all = 0, w_size_all = 0;   // composite: elements per row of the whole plan
+    int in_stride = 0, out_stride = 0, w_stride = 0;         // sub-plan: row strides in elements (0 = regular)
+    std::vector<int> in_base, out_base, w_base;              // sub-plan: element offset of input irrep i / output irrep i / path p
+    std::vector<std::pair<int, int>> zero_in;                // sub-plan: (offset, length) element runs of the whole input row that no path of
+                                                             // any class reads; its backward writes their zero rows of the per-edge workspace
+    int in_size() const { return !subs.empty() ? in_size_all : (in_stride ? in_stride : in_dim * C); }
+    int out_size() const { return !subs.empty() ? out_size_all : (out_stride ? out_stride : out_dim * C); }
+    int w_size() const { return !subs.empty() ? w_size_all : (w_stride ? w_stride : (int)paths.size() * C); }
+    int xoff(int i_in, int m1) const
+    {
+        if (!in_base.empty()) return in_base[i_in] + m1 * C;
+        int off = 0;
+        for (int i = 0; i < i_in; ++i) off += 2 * irreps_in[i].l + 1;
+        return (off + m1) * C;
+    }
+    int ooff(int i_out, int m3) const
+    {
+        if (!out_base.empty()) return out_base[i_out] + m3 * C;
+        int off = 0;
+        for (int i = 0; i < i_out; ++i) off += 2 * irreps_out[i].l + 1;
+        return (off + m3) * C;
+    }
+    int woff(int p) const { return w_base.empty() ? p * C : w_base[p]; }
 };
 
 namespace e3 {
@@ -111,6 +141,9 @@ double cg_real_host(int l1, int l2, int l3, int m1, int m2, int m3);   // same r
 int plan_build_tables(e3_plan &pl, const e3_irrep *irreps_in, int n_in, int sh_lmax, const e3_irrep *irreps_out,
                       int n_out, const e3_path *paths, int n_paths, e3_dtype dtype, bool cg_on_device);
 void plan_make_roles(e3_plan &pl);
+bool plan_is_composite(const e3_irrep *irreps_in, int n_in, const e3_irrep *irreps_out, int n_out);   // multiplicities differ
+int plan_build_composite(e3_plan &pl, const e3_irrep *irreps_in, int n_in, int sh_lmax, const e3_irrep *irreps_out, int n_out,
+                         const e3_path *paths, int n_paths, e3_dtype dtype, bool cg_on_device);
 
 // codegen.cpp
 std::string gen_forward_source(e3_plan &pl);    // also sets pl.fwd.smem_dyn

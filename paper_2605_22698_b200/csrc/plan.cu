@@ -260,6 +260,115 @@ int plan_build_tables(e3_plan &pl, const e3_irrep *irreps_in, int n_in, int sh_l
 }
 
 // ---------------------------------------------------------------------------------------------
+// NEXT-4 (NequIP's `64x0e + 64x0o + 32x1o + 32x1e + 32x2e + 32x2o`): per-irrep multiplicities.
+// A channelwise (uvu) path keeps the multiplicity of its input irrep, so the plan falls apart into MULTIPLICITY CLASSES that
+// share nothing but the edge's SH row: the composite holds one regular generated sub-plan per class, whose kernels address the
+// rows of the whole plan (block offsets and row strides overridden).  Layout (the oracle's orc_tp_mul_*): a node row is the
+// irrep blocks back to back, block i = (2l_i+1) x mul_i with index m*mul_i + u; a weights row is mul(p) values per path, paths
+// back to back.
+// ---------------------------------------------------------------------------------------------
+bool plan_is_composite(const e3_irrep *irreps_in, int n_in, const e3_irrep *irreps_out, int n_out)
+{
+    if (!irreps_in || !irreps_out || n_in < 1 || n_out < 1) return false;
+    for (int i = 0; i < n_in; ++i) if (irreps_in[i].mul != irreps_in[0].mul) return true;
+    for (int i = 0; i < n_out; ++i) if (irreps_out[i].mul != irreps_in[0].mul) return true;
+    return false;
+}
+
+int plan_build_composite(e3_plan &pl, const e3_irrep *irreps_in, int n_in, int sh_lmax, const e3_irrep *irreps_out, int n_out,
+                         const e3_path *paths, int n_paths, e3_dtype dtype, bool cg_on_device)
+{
+    if (!irreps_in || !irreps_out || !paths || n_in < 1 || n_out < 1 || n_paths < 1) {
+        set_error("plan: null or empty irreps / path table");
+        return E3_ERR_INVALID_ARG;
+    }
+    if (dtype != E3_F32 && dtype != E3_BF16) { set_error("plan: unknown dtype %d", (int)dtype); return E3_ERR_INVALID_ARG; }
+    if (sh_lmax < 0 || sh_lmax > kMaxL) { set_error("plan: sh_lmax %d not in 0..%d", sh_lmax, kMaxL); return E3_ERR_UNSUPPORTED; }
+    pl.irreps_in.assign(irreps_in, irreps_in + n_in);
+    pl.irreps_out.assign(irreps_out, irreps_out + n_out);
+    pl.sh_lmax = sh_lmax;
+    pl.sh_dim = (sh_lmax + 1) * (sh_lmax + 1);
+    pl.dtype = dtype;
+    pl.C = 0;
+    std::vector<int> in_base(n_in), out_base(n_out), w_base(n_paths);
+    pl.in_dim = pl.out_dim = 0;
+    pl.in_size_all = pl.out_size_all = pl.w_size_all = 0;
+    auto check = [&](const e3_irrep &r, const char *what, int i) {
+        if (r.l < 0 || (r.parity != 1 && r.parity != -1) || r.mul < 1) { set_error("plan: bad %s irrep %d", what, i); return (int)E3_ERR_INVALID_ARG; }
+        if (r.l > kMaxL) { set_error("plan: %s irrep %d has l=%d > %d", what, i, r.l, kMaxL); return (int)E3_ERR_UNSUPPORTED; }
+        if (r.mul % 4 != 0) { set_error("plan: unequal multiplicities must all be multiples of 4 (%s irrep %d has %d)", what, i, r.mul); return (int)E3_ERR_UNSUPPORTED; }
+        return (int)E3_OK;
+    };
+    for (int i = 0; i < n_in; ++i) {
+        if (int rc = check(irreps_in[i], "input", i)) return rc;
+        in_base[i] = pl.in_size_all;
+        pl.in_size_all += (2 * irreps_in[i].l + 1) * irreps_in[i].mul;
+        pl.in_dim += 2 * irreps_in[i].l + 1;
+    }
+    for (int i = 0; i < n_out; ++i) {
+        if (int rc = check(irreps_out[i], "output", i)) return rc;
+        out_base[i] = pl.out_size_all;
+        pl.out_size_all += (2 * irreps_out[i].l + 1) * irreps_out[i].mul;
+        pl.out_dim += 2 * irreps_out[i].l + 1;
+    }
+    std::vector<char> in_used(n_in, 0), out_fed(n_out, 0);
+    std::vector<int> classes;                       // multiplicities in order of first use by a path
+    for (int p = 0; p < n_paths; ++p) {
+        const e3_path &q = paths[p];
+        if (q.i_in < 0 || q.i_in >= n_in || q.i_out < 0 || q.i_out >= n_out || q.l_sh < 0 || q.l_sh > sh_lmax) {
+            set_error("plan: path %d has an index out of range", p);
+            return E3_ERR_BAD_PATH;
+        }
+        const int mul = irreps_in[q.i_in].mul;
+        if (irreps_out[q.i_out].mul != mul) {
+            set_error("plan: path %d joins an input irrep of multiplicity %d to an output irrep of multiplicity %d (a channelwise path keeps it)", p, mul, irreps_out[q.i_out].mul);
+            return E3_ERR_BAD_PATH;
+        }
+        w_base[p] = pl.w_size_all;
+        pl.w_size_all += mul;
+        in_used[q.i_in] = 1; out_fed[q.i_out] = 1;
+        if (std::find(classes.begin(), classes.end(), mul) == classes.end()) classes.push_back(mul);
+    }
+    pl.path_map.assign(n_paths, { 0, 0 });
+    for (size_t k = 0; k < classes.size(); ++k) {
+        const int mul = classes[k];
+        std::vector<e3_irrep> ii, io;
+        std::vector<int> gi, go;                    // sub-plan index -> index in the whole plan
+        std::vector<int> li(n_in, -1), lo(n_out, -1);
+        for (int i = 0; i < n_in; ++i) if (irreps_in[i].mul == mul && in_used[i]) { li[i] = (int)ii.size(); ii.push_back(irreps_in[i]); gi.push_back(i); }
+        // output blocks of this multiplicity that no path feeds are still written (zeros) by this class
+        for (int i = 0; i < n_out; ++i) if (irreps_out[i].mul == mul) { lo[i] = (int)io.size(); io.push_back(irreps_out[i]); go.push_back(i); out_fed[i] = 1; }
+        std::vector<e3_path> pp;
+        std::vector<int> gp;
+        for (int p = 0; p < n_paths; ++p)
+            if (irreps_in[paths[p].i_in].mul == mul) {
+                pl.path_map[p] = { (int)k, (int)pp.size() };
+                pp.push_back({ li[paths[p].i_in], paths[p].l_sh, lo[paths[p].i_out] });
+                gp.push_back(p);
+            }
+        e3_plan *sp = new (std::nothrow) e3_plan();
+        if (!sp) { set_error("out of host memory"); return E3_ERR_INVALID_ARG; }
+        pl.subs.push_back(sp);
+        int rc = plan_build_tables(*sp, ii.data(), (int)ii.size(), sh_lmax, io.data(), (int)io.size(), pp.data(), (int)pp.size(), dtype, cg_on_device);
+        if (rc != E3_OK) return rc;
+        sp->in_stride = pl.in_size_all; sp->out_stride = pl.out_size_all; sp->w_stride = pl.w_size_all;
+        for (int g : gi) sp->in_base.push_back(in_base[g]);
+        for (int g : go) sp->out_base.push_back(out_base[g]);
+        for (int g : gp) sp->w_base.push_back(w_base[g]);
+        pl.nnz_total += sp->nnz_total;
+    }
+    for (int i = 0; i < n_out; ++i)
+        if (!out_fed[i]) { set_error("plan: output irrep %d is fed by no path and no multiplicity class matches it", i); return E3_ERR_UNSUPPORTED; }
+    // input irreps no path reads: their rows of the per-edge grad_feats workspace are zeroed by the first class's backward
+    for (int i = 0; i < n_in; ++i)
+        if (!in_used[i]) pl.subs[0]->zero_in.push_back({ in_base[i], (2 * irreps_in[i].l + 1) * irreps_in[i].mul });
+    // the caller's path list, for e3_plan_get_cg / counting
+    pl.paths.clear();
+    for (int p = 0; p < n_paths; ++p) pl.paths.push_back(pl.subs[pl.path_map[p].first]->paths[pl.path_map[p].second]);
+    return E3_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
 // Forward roles: contiguous groups of output irreps (ordered by their first feeding path), each
 // owned by one warp.  Paths that add into the same output irrep (A6) always share a role.
 // ---------------------------------------------------------------------------------------------

@@ -1,0 +1,135 @@
+"""NEXT-4: plans with per-irrep multiplicities on the CUDA path (one generated kernel
+pair per multiplicity class over the rows of the whole plan) against the fp64 oracle's orc_tp_mul_* on the same inputs."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+import torch
+
+import oracle as O
+from helpers import TOL_BF16, TOL_FWD, TOL_VJP, relerr, to_dev
+from paper_2605_22698_b200 import binding as B
+from paper_2605_22698_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+NEQUIP = [(0, 1, 64), (0, -1, 64), (1, -1, 32), (1, 1, 32), (2, 1, 32), (2, -1, 32)]
+
+
+def _ragged_graph(rng, n, max_deg):
+    rcv, snd = [], []
+    for r in range(n):
+        d = int(rng.integers(0, max_deg + 1)) if r % 7 else 0              # isolated receivers included
+        s = np.sort(rng.integers(0, n, size=d))
+        rcv += [r] * d
+        snd += list(s)
+    return np.asarray(snd, np.int32), np.asarray(rcv, np.int32)
+
+
+def _case(irreps_in, sh_lmax, out_lmax, n, max_deg, seed, natural=False, drop_paths_of=None):
+    rng = np.random.default_rng(seed)
+    irreps_out, paths = O.all_paths(irreps_in, sh_lmax, out_lmax, natural)
+    if drop_paths_of is not None:                                            # an input irrep that no path reads
+        keep = [k for k, p in enumerate(paths) if p[0] != drop_paths_of]
+        irreps_out = [irreps_out[paths[k][2]] for k in keep]
+        paths = [(paths[k][0], paths[k][1], j) for j, k in enumerate(keep)]
+    in_size, sh_dim, out_size, w_size = O.tp_mul_dims(irreps_in, sh_lmax, irreps_out, paths)
+    snd, rcv = _ragged_graph(rng, n, max_deg)
+    e = len(snd)
+    vec = (rng.normal(size=(e, 3)) * 2).astype(np.float32)
+    x = rng.normal(size=(n, in_size)).astype(np.float32)
+    w = (rng.normal(size=(e, w_size)) / np.sqrt(len(paths))).astype(np.float32)
+    G = rng.normal(size=(n, out_size)).astype(np.float32)
+    return (irreps_in, sh_lmax, irreps_out, paths), (in_size, sh_dim, out_size, w_size), snd, rcv, vec, x, w, G
+
+
+def _run_both(pl, sizes, snd, rcv, vec, x, w, G, storage="f32"):
+    n = x.shape[0]
+    plan = B.e3_plan_create(*pl, B.E3_BF16 if storage == "bf16" else B.E3_F32)
+    assert (plan.feats_per_node, plan.sh_dim, plan.out_per_node, plan.weights_per_edge) == sizes
+    st = plan.storage
+    xs, ws = W.round_to_storage(x, storage), W.round_to_storage(w, storage)
+    sd, rd, vd = to_dev(snd), to_dev(rcv), to_dev(vec)
+    xd, wd, Gd = to_dev(xs, st), to_dev(ws, st), to_dev(G)
+    row_ptr, perm_s, col_ptr = B.e3_graph_prepare(sd, rd, n, validate=True)
+    sh = B.e3_sh_fwd(plan, vd)
+    out = torch.full((n, plan.out_per_node), float("nan"), device="cuda")
+    B.e3_tp_scatter_fwd(plan, xd, sh, wd, sd, rd, row_ptr, n, out=out)
+    dx, dY, dw = B.e3_tp_scatter_bwd(plan, xd, sh, wd, sd, rd, row_ptr, perm_s, col_ptr, n, Gd)
+    out2 = B.e3_tp_scatter_fwd(plan, xd, sh, wd, sd, rd, row_ptr, n)
+    dx2, dY2, dw2 = B.e3_tp_scatter_bwd(plan, xd, sh, wd, sd, rd, row_ptr, perm_s, col_ptr, n, Gd)
+    torch.cuda.synchronize()
+    assert torch.equal(out, out2) and torch.equal(dx, dx2) and torch.equal(dY, dY2) and torch.equal(dw, dw2)    # run-to-run bit-identical
+    Y = O.sh(pl[1], vec.astype(np.float64))
+    Yin = W.round_to_storage(Y, storage).astype(np.float64) if storage == "bf16" else Y
+    x64, w64 = np.asarray(xs, np.float64), np.asarray(ws, np.float64)
+    ref_out = O.tp_mul_fwd(*pl, x64, Yin, w64, snd, rcv, n)
+    ref = O.tp_mul_bwd(*pl, x64, Yin, w64, snd, rcv, n, G.astype(np.float64))
+    got = [t.float().cpu().numpy() for t in (out, dx, dY, dw)]
+    assert np.isfinite(got[0]).all()
+    errs = dict(out=relerr(got[0], ref_out), dx=relerr(got[1], ref[0]), dY=relerr(got[2], ref[1]), dw=relerr(got[3], ref[2]))
+    return plan, errs
+
+
+@pytest.mark.parametrize("irreps_in,lmax", [
+    (NEQUIP, 2),
+    ([(0, 1, 8), (0, -1, 8), (1, -1, 4), (1, 1, 4), (2, 1, 4), (2, -1, 4)], 2),                 # class 4 runs on the first-generation kernels
+    ([(0, 1, 128), (1, -1, 64), (2, 1, 32), (3, -1, 16)], 3),                                  # four classes, l up to 3
+    ([(0, 1, 64), (1, -1, 32), (1, 1, 64), (2, 1, 32)], 2),                                    # classes interleaved in the row
+])
+def test_unequal_multiplicities_against_the_oracle(irreps_in, lmax):
+    pl, sizes, *data = _case(irreps_in, lmax, lmax, n=37, max_deg=21, seed=len(irreps_in) + lmax)
+    plan, errs = _run_both(pl, sizes, *data)
+    print(plan.kernel_info(0), plan.kernel_info(1), {k: f"{v:.2e}" for k, v in errs.items()})
+    assert errs["out"] <= TOL_FWD and max(errs["dx"], errs["dY"], errs["dw"]) <= TOL_VJP, errs
+
+
+def test_unequal_multiplicities_bf16_storage():
+    pl, sizes, *data = _case(NEQUIP, 2, 2, n=23, max_deg=15, seed=11)
+    _, errs = _run_both(pl, sizes, *data, storage="bf16")
+    assert max(errs.values()) <= TOL_BF16, errs
+
+
+def test_input_irrep_without_paths_and_natural_parity():
+    # the 2o block (index 5) is read by no path: its grad_feats rows must come out as exact zeros
+    pl, sizes, *data = _case(NEQUIP, 2, 2, n=19, max_deg=9, seed=5, drop_paths_of=5)
+    _, errs = _run_both(pl, sizes, *data)
+    assert errs["out"] <= TOL_FWD and max(errs["dx"], errs["dY"], errs["dw"]) <= TOL_VJP, errs
+    pl, sizes, *data = _case(NEQUIP, 2, 2, n=19, max_deg=9, seed=6, natural=True)
+    _, errs = _run_both(pl, sizes, *data)
+    assert errs["out"] <= TOL_FWD and max(errs["dx"], errs["dY"], errs["dw"]) <= TOL_VJP, errs
+
+
+def test_composite_plan_rejections_and_cg_table():
+    with pytest.raises(B.E3Error):                                           # a path may not change the multiplicity
+        B.e3_plan_create([(0, 1, 8), (1, -1, 4)], 1, [(1, -1, 8)], [(0, 1, 0), (1, 0, 0)])
+    with pytest.raises(B.E3Error):                                           # multiplicities must be multiples of 4
+        B.e3_plan_create([(0, 1, 8), (1, -1, 6)], 1, [(0, 1, 8), (1, -1, 6)], [(0, 0, 0), (1, 0, 1)])
+    irreps_out, paths = O.all_paths(NEQUIP, 2, 2)
+    plan = B.e3_plan_create(NEQUIP, 2, irreps_out, paths)
+    for p in (0, 7, len(paths) - 1):                                         # e3_plan_get_cg follows the caller's path numbering
+        l1, l2, l3 = NEQUIP[paths[p][0]][0], paths[p][1], irreps_out[paths[p][2]][0]
+        dense = np.zeros((2 * l1 + 1, 2 * l2 + 1, 2 * l3 + 1))
+        for m1, m2, m3, c in plan.get_cg(p):
+            dense[m1, m2, m3] = c
+        assert np.abs(dense - O.cg_real(l1, l2, l3)).max() < 1e-14
+
+
+def test_session_host_path_with_unequal_multiplicities():
+    pl, sizes, snd, rcv, vec, x, w, G = _case(NEQUIP, 2, 2, n=41, max_deg=17, seed=9)
+    n, e = x.shape[0], len(snd)
+    plan = B.e3_plan_create(*pl)
+    sess = B.Session(plan, e, n)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    hout = torch.empty((n, plan.out_per_node), dtype=torch.float32).pin_memory()
+    hdx = torch.empty((n, plan.feats_per_node), dtype=torch.float32).pin_memory()
+    hdw = torch.empty((e, plan.weights_per_edge), dtype=torch.float32).pin_memory()
+    hF = torch.empty((n, 3), dtype=torch.float32).pin_memory()
+    sess.run_host(pin(vec), pin(x), pin(w), pin(snd), pin(rcv), n, grad_out=pin(G), out=hout, grad_feats=hdx, grad_weights=hdw, forces=hF)
+    Y = O.sh(2, vec.astype(np.float64))
+    ref_out = O.tp_mul_fwd(*pl, x.astype(np.float64), Y, w.astype(np.float64), snd, rcv, n)
+    dx, dY, dw = O.tp_mul_bwd(*pl, x.astype(np.float64), Y, w.astype(np.float64), snd, rcv, n, G.astype(np.float64))
+    F = O.force_reduce(O.sh_bwd(2, vec.astype(np.float64), dY), snd, rcv, n)
+    assert relerr(hout.numpy(), ref_out) <= TOL_FWD
+    assert relerr(hdx.numpy(), dx) <= TOL_VJP and relerr(hdw.numpy(), dw) <= TOL_VJP
+    assert relerr(hF.numpy(), F) <= TOL_VJP

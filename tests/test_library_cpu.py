@@ -60,9 +60,24 @@ def test_jit_check_rejects_bad_plans():
     with pytest.raises(B.E3Error) as e:        # l > 3
         B.e3_jit_check([(4, 1, C)], 1, [(4, 1, C)], [(0, 0, 0)])
     assert e.value.status == B.E3_ERR_UNSUPPORTED
-    with pytest.raises(B.E3Error) as e:        # unequal multiplicities
-        B.e3_jit_check([(0, 1, C), (1, -1, 2 * C)], 1, [(0, 1, C)], [(0, 0, 0)])
+    with pytest.raises(B.E3Error) as e:        # unequal multiplicities that are not multiples of 4
+        B.e3_jit_check([(0, 1, 8), (1, -1, 6)], 1, [(0, 1, 8), (1, -1, 6)], [(0, 0, 0), (1, 0, 1)])
     assert e.value.status == B.E3_ERR_UNSUPPORTED
+    with pytest.raises(B.E3Error) as e:        # a channelwise path cannot change the multiplicity
+        B.e3_jit_check([(0, 1, 8), (1, -1, 4)], 1, [(1, -1, 8)], [(0, 1, 0), (1, 0, 0)])
+    assert e.value.status == B.E3_ERR_BAD_PATH
+
+
+def test_jit_check_compiles_the_papers_nequip_irreps():
+    """NEXT-4: PAPER.md L484-L485 `64x0e + 64x0o + 32x1o + 32x1e + 32x2e + 32x2o` (l_max 2, L486) is one kernel pair per
+    multiplicity class; an input irrep that no path reads is allowed."""
+    ii = [(0, 1, 64), (0, -1, 64), (1, -1, 32), (1, 1, 32), (2, 1, 32), (2, -1, 32)]
+    io, pp = B.e3_all_paths(ii, 2, 2)
+    assert len(pp) == 30 and all(io[k][2] == ii[p[0]][2] for k, p in enumerate(pp))
+    r = B.e3_jit_check(ii, 2, io, pp, B.E3_F32)
+    assert r["fwd_regs"] > 0 and r["bwd_regs"] > 0 and r["fwd_spill"] <= 64 and r["bwd_spill"] <= 64, r
+    r = B.e3_jit_check([(0, 1, 4), (1, -1, 8)], 1, [(0, 1, 4)], [(0, 0, 0)])
+    assert r["fwd_regs"] > 0
 
 
 @pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-device behaviour")
