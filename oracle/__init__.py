@@ -388,13 +388,15 @@ def symcon2_bwd(irreps_in, irreps_out, paths, n_species, A, species, W, g):
 # deployment to larger systems"; L298 / L497 cutoff 5 A): neighbour list and receiver-range sharding.  Plain numpy, brute force.
 # The paper prints neither, so both are readings (N1, N2).
 # ------------------------------------------------------------------------------------------------------------------
-def neighbor_build(pos, box, cutoff):
+def neighbor_build(pos, box, cutoff, only_receivers=None):
     """Reading N1.  All pairs, no cell list.  The inclusion test decides an integer (which edges exist), so it is taken in
     the kernel's precision, IEEE float32 with every operation rounded (no fused multiply-add):
         d_a = pos[r,a] - pos[s,a];  if box_a > 0:  d_a = d_a - box_a * rint(d_a / box_a)          (minimum image, reading A10)
         d2  = (d_x*d_x + d_y*d_y) + d_z*d_z;   edge s -> r  iff  s != r and d2 < cutoff*cutoff        (strict, reading A11)
     box_a = 0 means no periodicity along a; a periodic box_a must be >= 2*cutoff (one image at most).  Edges are ordered by
     receiver, ties by ascending sender (A11).  Returns senders, receivers (int32), vec [E,3] float32 (= d) and row_ptr.
+    `only_receivers` (ascending atom ids) restricts the OUTPUT to the in-edges of those atoms (sampling for large systems; row_ptr
+    is then None); the arithmetic is unchanged.
     Pins (tests/test_oracle_nb.py): scipy's cKDTree on the same positions, the simple cubic lattice's coordination numbers,
     pair symmetry, python-loop brute force on an open cluster, the harness graph of config 1."""
     pos = np.ascontiguousarray(pos, dtype=np.float32)
@@ -405,20 +407,24 @@ def neighbor_build(pos, box, cutoff):
     rc2 = rc * rc
     n = pos.shape[0]
     snd, rcv, vec = [], [], []
-    for r0 in range(0, n, 256):                                   # receivers in slabs only to bound memory
-        pr = pos[r0:r0 + 256]
+    rows = np.arange(n) if only_receivers is None else np.asarray(only_receivers, dtype=np.int64)
+    for r0 in range(0, len(rows), 256):                           # receivers in slabs only to bound memory
+        rid = rows[r0:r0 + 256]
+        pr = pos[rid]
         d = pr[:, None, :] - pos[None, :, :]                       # [R, N, 3] float32
         for a in range(3):
             if box[a] > 0:
                 d[:, :, a] = d[:, :, a] - box[a] * np.rint(d[:, :, a] / box[a])
         d2 = (d[:, :, 0] * d[:, :, 0] + d[:, :, 1] * d[:, :, 1]) + d[:, :, 2] * d[:, :, 2]
         keep = d2 < rc2
-        keep[np.arange(pr.shape[0]), np.arange(r0, r0 + pr.shape[0])] = False
+        keep[np.arange(pr.shape[0]), rid] = False
         rr, ss = np.nonzero(keep)                                  # row-major: receiver ascending, then sender ascending
-        rcv.append(rr + r0); snd.append(ss); vec.append(d[rr, ss])
+        rcv.append(rid[rr]); snd.append(ss); vec.append(d[rr, ss])
     snd = np.concatenate(snd).astype(np.int32) if snd else np.zeros(0, np.int32)
     rcv = np.concatenate(rcv).astype(np.int32) if rcv else np.zeros(0, np.int32)
     vec = np.concatenate(vec).astype(np.float32) if vec else np.zeros((0, 3), np.float32)
+    if only_receivers is not None:
+        return snd, rcv, vec, None
     row_ptr = np.zeros(n + 1, np.int32)
     np.add.at(row_ptr, rcv + 1, 1)
     return snd, rcv, vec, np.cumsum(row_ptr).astype(np.int32)

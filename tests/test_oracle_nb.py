@@ -49,6 +49,10 @@ def test_neighbor_oracle_matches_kdtree_away_from_the_cutoff(n, box, seed):
     assert np.all(np.diff(r) >= 0) and np.all((np.diff(s) > 0) | (np.diff(r) > 0))      # (receiver, sender) strictly ascending
     assert not np.any(s == r)
     assert np.array_equal(row_ptr, np.searchsorted(r, np.arange(n + 1), "left"))
+    pick = np.array([0, 7, n // 2, n - 1])                    # the sampled form returns exactly those receivers' rows
+    s1, r1, v1, _ = O.neighbor_build(pos, bx, 5.0, only_receivers=pick)
+    m = np.isin(r, pick)
+    assert np.array_equal(s1, s[m]) and np.array_equal(r1, r[m]) and np.array_equal(v1, vec[m])
 
 
 def test_neighbor_oracle_simple_cubic_coordination_numbers():
