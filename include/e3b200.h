@@ -291,6 +291,41 @@ int e3_symcon_bwd(const e3_symcon *sc, const float *feats, const int32_t *specie
                   const float *grad_out, float *grad_feats, float *grad_weights, void *workspace, size_t workspace_bytes,
                   e3_stream stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * NEXT-4: neighbour list on the device.  PAPER.md L66 (the Graph class computes edge vectors from positions and
+ * connectivity), L82 ("scale model deployment to larger systems"), L298 / L497 (5 A cutoff).  No formula is printed; reading N1
+ * (DESIGN.md), evaluated in float32 with every operation rounded (no fused multiply-add) so that the edge set is unique:
+ *   d_a = pos[r,a] - pos[s,a];   if box[a] > 0:  d_a = d_a - box[a] * rint(d_a / box[a])      (minimum image, reading A10)
+ *   d2 = (d_x*d_x + d_y*d_y) + d_z*d_z;   edge s -> r  iff  s != r  and  d2 < cutoff*cutoff     (strict, reading A11)
+ * Output, ordered by receiver with ties in ascending sender (A11), i.e. exactly what e3_tp_scatter_* expect:
+ *   senders[E], receivers[E] (int32), vec[E,3] = d (float), row_ptr[N+1] (= the row_ptr of e3_graph_prepare).
+ * pos [N,3] float on the device (any values; periodic axes are wrapped); box[3] on the HOST: edge length of a periodic axis, or 0
+ * for an open axis; a periodic edge shorter than 2*cutoff is E3_ERR_UNSUPPORTED (a sender would have two images in range).
+ * *n_edges (HOST) receives the edge count; if it exceeds max_edges (the capacity of senders / receivers / vec) nothing is written
+ * to them and E3_ERR_WORKSPACE is returned with *n_edges set, so the caller can allocate and call again.  Uses a cell list
+ * (integer atomics only); synchronises `stream` (the count is read back).  workspace >= e3_neighbor_workspace_bytes(n_nodes).
+ * -------------------------------------------------------------------------------------------*/
+size_t e3_neighbor_workspace_bytes(int32_t n_nodes);
+int e3_neighbor_build(const float *pos /*[N,3]*/, int32_t n_nodes, const float *box /*[3], host*/, float cutoff, int64_t max_edges,
+                      int32_t *senders, int32_t *receivers, float *vec /*[E,3]*/, int32_t *row_ptr /*[N+1]*/, int64_t *n_edges /*host*/,
+                      void *workspace, size_t workspace_bytes, e3_stream stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * NEXT-4 / SURVEY 8(e): receiver-range sharding of one graph over the GPUs of a node (HOST-side planning; all pointers are host
+ * pointers, no device work).  PAPER.md L82; reading N2.  Rank k owns the atoms [bounds[k], bounds[k+1]) and all their
+ * in-edges: boundary k is the receiver of edge floor(k*E/world) (n_nodes when that index is E), boundaries made non-decreasing,
+ * so the ranks hold about equal edge counts.  receivers must be ascending (E3_ERR_UNSORTED).
+ * e3_shard_localize describes the local problem of the owner of [lo, hi): its edge range [*e_lo, *e_hi), its halo (the senders
+ * of its edges that it does not own, ascending global ids, *n_halo of them) and its edges with LOCAL node ids: owned atoms are
+ * 0 .. hi-lo-1 in order, halo atoms follow in halo order.  halo, senders_local and receivers_local need room for *e_hi - *e_lo
+ * entries; pass the three of them and n_halo as NULL to query the edge range first.  The local problem is an ordinary
+ * e3_tp_scatter_fwd / _bwd call on hi-lo+n_halo nodes; paper_2605_22698_b200/sharded.py does the two exchanges with
+ * torch.distributed (halo rows of feats in, halo rows of grad_feats back, added in rank order).
+ * -------------------------------------------------------------------------------------------*/
+int e3_shard_ranges(const int32_t *receivers_h, int64_t n_edges, int32_t n_nodes, int world, int32_t *bounds /*[world+1]*/);
+int e3_shard_localize(const int32_t *senders_h, const int32_t *receivers_h, int64_t n_edges, int32_t n_nodes, int32_t lo, int32_t hi,
+                      int64_t *e_lo, int64_t *e_hi, int32_t *halo, int32_t *n_halo, int32_t *senders_local, int32_t *receivers_local);
+
 #ifdef __cplusplus
 }
 #endif

@@ -10,6 +10,7 @@ from __future__ import annotations
 import ctypes as C
 import os
 
+import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -25,6 +26,7 @@ SYMBOLS = [
     "e3_force_reduce", "e3_profile_set_mid_event", "e3_measure_fp32_peak", "e3_session_create", "e3_session_destroy", "e3_session_run_host",
     "e3_vjp_vjp_workspace_bytes", "e3_tp_scatter_vjp_vjp", "e3_sh_bwd_bwd",
     "e3_symcon_create", "e3_symcon_destroy", "e3_symcon_dims", "e3_symcon_fwd", "e3_symcon_workspace_bytes", "e3_symcon_bwd",
+    "e3_neighbor_workspace_bytes", "e3_neighbor_build", "e3_shard_ranges", "e3_shard_localize",
     "e3_radial_create", "e3_radial_destroy", "e3_radial_workspace_bytes", "e3_radial_weights_fwd", "e3_radial_weights_bwd",
 ]
 
@@ -63,6 +65,8 @@ def lib():
         L.e3_vjp_vjp_workspace_bytes.argtypes = [C.c_void_p, C.c_int64, C.c_int32]
         L.e3_symcon_workspace_bytes.restype = C.c_size_t
         L.e3_symcon_workspace_bytes.argtypes = [C.c_void_p, C.c_int32]
+        L.e3_neighbor_workspace_bytes.restype = C.c_size_t
+        L.e3_neighbor_workspace_bytes.argtypes = [C.c_int32]
         L.e3_radial_workspace_bytes.restype = C.c_size_t
         L.e3_radial_workspace_bytes.argtypes = [C.c_void_p, C.c_int64]
         _lib = L
@@ -420,3 +424,54 @@ class SymCon:
             self.destroy()
         except Exception:
             pass
+
+
+def e3_neighbor_build(pos, box, cutoff, max_edges=None, stream=None):
+    """pos: [N,3] float32 device tensor; box: three host floats (0 = open axis).  Returns senders, receivers, vec, row_ptr.
+    Without max_edges the call is made twice when the first capacity guess (64 edges per atom) is too small."""
+    _dev(pos, torch.float32)
+    N, dev = pos.shape[0], pos.device
+    bx = (C.c_float * 3)(*[float(b) for b in box])
+    nbytes = int(lib().e3_neighbor_workspace_bytes(C.c_int32(N)))
+    ws = torch.empty(max(nbytes, 1), dtype=torch.uint8, device=dev)
+    row_ptr = torch.empty(N + 1, dtype=torch.int32, device=dev)
+    cap = int(max_edges) if max_edges is not None else 64 * N
+    for attempt in range(2):
+        snd = torch.empty(max(cap, 1), dtype=torch.int32, device=dev)
+        rcv = torch.empty(max(cap, 1), dtype=torch.int32, device=dev)
+        vec = torch.empty((max(cap, 1), 3), dtype=torch.float32, device=dev)
+        n = C.c_int64(0)
+        rc = lib().e3_neighbor_build(_ptr(pos), C.c_int32(N), bx, C.c_float(float(cutoff)), C.c_int64(cap), _ptr(snd), _ptr(rcv), _ptr(vec),
+                                     _ptr(row_ptr), C.byref(n), _ptr(ws), C.c_size_t(ws.numel()), _stream(stream))
+        if rc == E3_ERR_WORKSPACE and n.value > cap and max_edges is None and attempt == 0:
+            cap = int(n.value)
+            continue
+        _check(rc, "e3_neighbor_build")
+        E = int(n.value)
+        return snd[:E], rcv[:E], vec[:E], row_ptr
+
+
+def _hptr(a, dtype):
+    assert isinstance(a, np.ndarray) and a.dtype == dtype and a.flags.c_contiguous
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def e3_shard_ranges(receivers_h, n_nodes, world):
+    """HOST numpy int32 receivers (ascending) -> list of world+1 atom boundaries."""
+    b = np.empty(world + 1, dtype=np.int32)
+    _check(lib().e3_shard_ranges(_hptr(receivers_h, np.int32), C.c_int64(receivers_h.shape[0]), C.c_int32(n_nodes), C.c_int(world),
+                                 _hptr(b, np.int32)), "e3_shard_ranges")
+    return [int(v) for v in b]
+
+
+def e3_shard_localize(senders_h, receivers_h, n_nodes, lo, hi):
+    """HOST numpy int32 index arrays -> dict(lo, hi, e_lo, e_hi, halo, senders_local, receivers_local) of the owner of [lo, hi)."""
+    e_lo, e_hi, nh = C.c_int64(), C.c_int64(), C.c_int32()
+    E = receivers_h.shape[0]
+    args = (_hptr(senders_h, np.int32), _hptr(receivers_h, np.int32), C.c_int64(E), C.c_int32(n_nodes), C.c_int32(lo), C.c_int32(hi))
+    _check(lib().e3_shard_localize(*args, C.byref(e_lo), C.byref(e_hi), None, None, None, None), "e3_shard_localize")
+    n = e_hi.value - e_lo.value
+    halo, sl, rl = (np.empty(max(n, 1), dtype=np.int32) for _ in range(3))
+    _check(lib().e3_shard_localize(*args, C.byref(e_lo), C.byref(e_hi), _hptr(halo, np.int32), C.byref(nh), _hptr(sl, np.int32),
+                                   _hptr(rl, np.int32)), "e3_shard_localize")
+    return dict(lo=lo, hi=hi, e_lo=e_lo.value, e_hi=e_hi.value, halo=halo[:nh.value].copy(), senders_local=sl[:n], receivers_local=rl[:n])

@@ -175,6 +175,7 @@ int launch_gsh_reduce(const float *parts, int n_parts, int64_t n, float *gsh, cu
 int measure_fp32_peak(double *tflops, double ms_target, cudaStream_t st);
 int launch_sh_bwd_bwd(int lmax, const float *vec, const float *gsh, const float *u, int64_t E, float *g_vec, float *g_sh, cudaStream_t st);
 int launch_add_inplace(float *dst, const float *src, long long n, cudaStream_t st);
+int launch_scan_i32(int32_t *ptr, int32_t n, int32_t *cursor, cudaStream_t st);   // ptr[0..n) -> inclusive scan in place; cursor[i] = ptr[i], i < n-1
 int launch_cg_planner(const int *triples /*[n,3] host*/, int n, std::vector<std::vector<double>> &dense_out);
 
 }  // namespace e3

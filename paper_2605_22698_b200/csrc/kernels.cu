@@ -334,6 +334,15 @@ __global__ void __launch_bounds__(1024) graph_scan_kernel(int32_t *__restrict__ 
     }
 }
 
+// exclusive-pointer scan used by the neighbour build (neighbor.cu): in-place inclusive scan of ptr[0..n) with ptr[0] = 0
+int launch_scan_i32(int32_t *ptr, int32_t n, int32_t *cursor, cudaStream_t st)
+{
+    if (n <= 0) return E3_OK;
+    graph_scan_kernel<<<1, 1024, 0, st>>>(ptr, n, cursor);
+    E3_CUDA_TRY(cudaGetLastError());
+    return E3_OK;
+}
+
 __global__ void graph_fill_kernel(const int32_t *__restrict__ snd, int64_t E, int32_t *__restrict__ cursor,
                                   int32_t *__restrict__ fill)
 {
