@@ -315,24 +315,27 @@ __device__ __forceinline__ void epilogue_tile(uint32_t tmem_d, int warp8, int la
 #define TILE_ROW(j) ((j) * 16 + (warp >> 2) * 8 + (lane & 7))
 #define TILE_QUAD() ((warp & 3) * 4 + (lane >> 3))
 
-// FORWARD, features as the M dimension:  D[f, e] = sum_k W3T[n_base + f, k] * h2[e, k]  for a slab of 128 output features (A operand,
-// staged once per CTA) and a run of 128-edge tiles (B operand = the rows of h2, already split into TF32 high / low parts by the hidden
-// kernel, brought in by 16-byte cp.async straight into the canonical layout, double-buffered).  In TMEM a lane is a FEATURE and a
-// column an EDGE, so a tcgen05.ld leaves every warp with 32 consecutive features of one edge per register: each store instruction
-// writes one full 128-byte line of w[e, n_base + 32 q ..] -- no shared-memory transpose.  While the eight warps drain tile i - 1, the
-// tensor core computes tile i (second TMEM buffer) and the copies of tile i + 1 are in flight.
-__global__ void __launch_bounds__(256, 1) radial_gemm_fwd_kernel(const float *__restrict__ Hhi, const float *__restrict__ Hlo, const float *__restrict__ W3Thi,
+// FORWARD, features as the M dimension:  D[f, e] = sum_k W3T[n_base + f, k] * h2[e, k]  for TWO slabs of 128 output features (A
+// operands, staged once per CTA, 128 KB with their high / low parts) and a run of 64-edge tiles (B operand = the rows of h2, already
+// split into TF32 high / low parts by the hidden kernel, brought in by 16-byte cp.async straight into the canonical layout).  Every B
+// tile (32 KB through the L2 -> SM crossbar) now feeds 64 KB of output: the first version of this kernel kept one slab and a
+// double-buffered B and was bound by exactly that traffic (91 GB of operand reads for 45.5 GB of output on config 4, every stall on
+// an address register waiting for the LSU queue to drain, profiles/r02b).  In TMEM a lane is a FEATURE and a column an EDGE, so a
+// tcgen05.ld leaves every warp with 32 consecutive features of one edge per register: each store instruction writes one full 128-byte
+// line of w[e, n_base + ..] -- no shared-memory transpose.  Tiles are 64 edges so that B (2 x 32 KB) AND TMEM (2 x 128 columns) are
+// double-buffered beside the 128 KB of slabs: the tensor core computes tile i while the eight warps drain tile i - 1 and the copies of
+// tile i + 1 are in flight; one __syncthreads and one mbarrier wait per tile.
+__global__ void __launch_bounds__(288, 1) radial_gemm_fwd_kernel(const float *__restrict__ Hhi, const float *__restrict__ Hlo, const float *__restrict__ W3Thi,
                                                                  const float *__restrict__ W3Tlo, float *__restrict__ D, long long ldd, long long E, int N,
                                                                  int tiles_per_cta, int nprod)
 {
-    constexpr int NT = 128;                                                  // edges per tile (MMA N)
-    extern __shared__ __align__(1024) unsigned char smem[];
-    unsigned char *sAhi = smem, *sAlo = smem + 32768;                       // the feature slab [128 x 64], high / low
-    unsigned char *sB = smem + 65536;                                       // 2 buffers x (hi 32 KB, lo 32 KB)
+    constexpr int NT = 64;                                                   // edges per tile (MMA N)
+    extern __shared__ __align__(1024) unsigned char smem[];                  // [slab 0 hi | slab 0 lo | slab 1 hi | slab 1 lo] 32 KB each, then 2 x [B hi | B lo] 16 KB each
     __shared__ __align__(8) unsigned long long mbar[2];
     __shared__ uint32_t tmem_base_s;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int n_base = blockIdx.x * kTileM;
+    const int n_base = blockIdx.x * (2 * kTileM);
+    const bool two = n_base + kTileM < N;                                    // the second slab holds features
     const long long n_etiles = (E + NT - 1) / NT;
     const long long t_begin = (long long)blockIdx.y * tiles_per_cta;
     const long long t_end = t_begin + tiles_per_cta < n_etiles ? t_begin + tiles_per_cta : n_etiles;
@@ -347,22 +350,29 @@ __global__ void __launch_bounds__(256, 1) radial_gemm_fwd_kernel(const float *__
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(mbar_s + 8) : "memory");
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    const uint32_t sAhi_s = (uint32_t)__cvta_generic_to_shared(sAhi), sAlo_s = sAhi_s + 32768, sB_s = sAhi_s + 65536;
-    // stationary operand: 128 rows of W3^T (zero beyond N), high and low parts
+    const uint32_t sA_s = (uint32_t)__cvta_generic_to_shared(smem), sB_s = sA_s + 131072;
+    // warps 0-7 copy operands and drain TMEM; warp 8 only issues the MMAs (a ninth warp, so that no draining warp starts late)
+    const bool worker = warp < 8;
+    // stationary operands: 2 x 128 rows of W3^T (zero beyond N), high and low parts
+    if (worker)
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
-        const int row = TILE_ROW(j), q = TILE_QUAD();
-        const uint32_t off = canon_off(row, q * 4);
-        const bool v = n_base + row < N;
-        const float *sh_ = W3Thi + (long long)(v ? n_base + row : 0) * kH + q * 4, *sl_ = W3Tlo + (long long)(v ? n_base + row : 0) * kH + q * 4;
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(sAhi_s + off), "l"(sh_), "r"(v ? 16 : 0) : "memory");
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(sAlo_s + off), "l"(sl_), "r"(v ? 16 : 0) : "memory");
-    }
-    auto issue_b = [&](long long t, int buf) {
-        const long long e0 = t * NT;
-        const uint32_t bh = sB_s + buf * 65536, bl = bh + 32768;
+    for (int sl = 0; sl < 2; ++sl)
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
+            const int row = TILE_ROW(j), q = TILE_QUAD();
+            const uint32_t off = sl * 65536 + canon_off(row, q * 4);
+            const int f = n_base + sl * kTileM + row;
+            const bool v = f < N;
+            const float *sh_ = W3Thi + (long long)(v ? f : 0) * kH + q * 4, *sl_ = W3Tlo + (long long)(v ? f : 0) * kH + q * 4;
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(sA_s + off), "l"(sh_), "r"(v ? 16 : 0) : "memory");
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(sA_s + 32768 + off), "l"(sl_), "r"(v ? 16 : 0) : "memory");
+        }
+    auto issue_b = [&](long long t, int buf) {
+        if (!worker) return;
+        const long long e0 = t * NT;
+        const uint32_t bh = sB_s + buf * 32768, bl = bh + 16384;
+#pragma unroll
+        for (int j = 0; j < NT / 16; ++j) {
             const int row = TILE_ROW(j), q = TILE_QUAD();
             const uint32_t off = canon_off(row, q * 4);
             const bool v = e0 + row < E;
@@ -378,13 +388,16 @@ __global__ void __launch_bounds__(256, 1) radial_gemm_fwd_kernel(const float *__
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem = tmem_base_s;
     const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(NT >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
-    const int feat = n_base + (warp & 3) * 32 + lane;                       // this thread's output column of w
+    // warp -> (slab, TMEM lane quarter): it drains the 64 edge columns of its 32 features in two 32-column blocks
+    const int slab = warp >> 2, quarter = warp & 3;
+    const int feat = n_base + slab * kTileM + quarter * 32 + lane;           // this thread's output column of w
     auto epilogue = [&](long long t, int buf) {
         const long long e0 = t * NT;
+        if (!worker || (slab == 1 && !two)) return;                          // warp-uniform
 #pragma unroll 1
-        for (int c0 = (warp >> 2) * (NT / 2); c0 < (warp >> 2) * (NT / 2) + NT / 2; c0 += 32) {
+        for (int c0 = 0; c0 < NT; c0 += 32) {
             uint32_t v[32];
-            const uint32_t taddr = tmem + buf * NT + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)c0;
+            const uint32_t taddr = tmem + buf * 128 + slab * 64 + ((uint32_t)(quarter * 32) << 16) + (uint32_t)c0;
             asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
                          "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
                          "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
@@ -410,30 +423,30 @@ __global__ void __launch_bounds__(256, 1) radial_gemm_fwd_kernel(const float *__
     uint32_t ph0 = 0, ph1 = 0;
     for (long long t = t_begin; t < t_end; ++t) {
         const int i = (int)(t - t_begin), buf = i & 1;
-        asm volatile("cp.async.wait_group 0;" ::: "memory");                 // tile t (and, the first time, the slab) has landed
+        // B[buf ^ 1] was last read by the MMAs of tile t - 1, whose completion every thread has waited for: refill it now, so that the
+        // copies of tile t + 1 are in flight during the MMAs of tile t and the drain of tile t - 1
+        if (t + 1 < t_end) {
+            issue_b(t + 1, buf ^ 1);
+            asm volatile("cp.async.wait_group 1;" ::: "memory");             // tile t (and, the first time, the slabs) has landed
+        } else {
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+        }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-        __syncthreads();
-        if (tid == 0) {
+        __syncthreads();                                                     // also: every warp has drained TMEM buffer `buf` (tile t - 2)
+        if (tid == 256) {
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            issue_chunk(tmem + buf * NT, sAhi_s, sAlo_s, sB_s + buf * 65536, sB_s + buf * 65536 + 32768, idesc, true, nprod);
+            const uint32_t bh = sB_s + buf * 32768, bl = bh + 16384;
+            issue_chunk(tmem + buf * 128, sA_s, sA_s + 32768, bh, bl, idesc, true, nprod);
+            if (two) issue_chunk(tmem + buf * 128 + 64, sA_s + 65536, sA_s + 98304, bh, bl, idesc, true, nprod);
             asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(mbar_s + buf * 8) : "memory");
         }
-        if (i > 0) {                                     // tile t - 1: its MMAs are done -> its operand buffer is free, its accumulators ready
-            const int pb = buf ^ 1;
-            mbar_wait_parity(mbar_s + pb * 8, pb ? ph1 : ph0);
-            if (pb) ph1 ^= 1u; else ph0 ^= 1u;
-            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        }
-        if (t + 1 < t_end) issue_b(t + 1, buf ^ 1);      // in flight while tile t - 1 drains and the tensor core works on tile t
-        if (i > 0) epilogue(t - 1, buf ^ 1);
-    }
-    {
-        const int pb = (int)((t_end - 1 - t_begin) & 1);
-        mbar_wait_parity(mbar_s + pb * 8, pb ? ph1 : ph0);
+        if (i > 0) epilogue(t - 1, buf ^ 1);             // overlaps the MMAs of tile t
+        mbar_wait_parity(mbar_s + buf * 8, buf ? ph1 : ph0);                 // tile t: MMAs done -> B[buf] is free, its accumulators are ready
+        if (buf) ph1 ^= 1u; else ph0 ^= 1u;
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        epilogue(t_end - 1, pb);
     }
+    epilogue(t_end - 1, (int)((t_end - 1 - t_begin) & 1));
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 256;" :: "r"(tmem) : "memory");
@@ -542,7 +555,7 @@ __global__ void __launch_bounds__(256, 1) radial_gemm_bwd_kernel(const float *__
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 64;" :: "r"(tmem) : "memory");
 }
 
-constexpr int kGemmSmem = 196608;      // forward: A 64 KB + 2 x 64 KB of B; backward: 2 x 96 KB stages (the epilogue stages through an idle buffer)
+constexpr int kGemmSmem = 196608;      // forward: 2 x 64 KB of A + 64 KB of B; backward: 2 x 96 KB stages (the epilogue stages through an idle buffer)
 
 int launch_gemm_fwd(const float *Hhi, const float *Hlo, const float *W3Thi, const float *W3Tlo, float *D, long long ldd, long long E, int N, cudaStream_t st)
 {
@@ -553,17 +566,17 @@ int launch_gemm_fwd(const float *Hhi, const float *Hlo, const float *W3Thi, cons
         attr_set = true;
     }
     if (E <= 0) return E3_OK;
-    // grid: (feature slabs of 128) x (runs of edge tiles): a CTA keeps its slab for `tiles_per_cta` 128-edge tiles; enough CTAs for
+    // grid: (pairs of 128-feature slabs) x (runs of edge tiles): a CTA keeps its slabs for `tiles_per_cta` 64-edge tiles; enough CTAs for
     // ~8 per SM so that the slabs of one edge range run together (the h2 rows they share stay in L2)
-    const int slabs = (N + kTileM - 1) / kTileM;
-    const long long n_etiles = (E + 127) / 128;
+    const int slabs = (N + 2 * kTileM - 1) / (2 * kTileM);       // pairs of 128-feature slabs
+    const long long n_etiles = (E + 63) / 64;
     long long runs = (148LL * 8 + slabs - 1) / slabs;
     if (runs > n_etiles) runs = n_etiles;
     const int tiles_per_cta = (int)((n_etiles + runs - 1) / runs);
     runs = (n_etiles + tiles_per_cta - 1) / tiles_per_cta;
     if (runs > 65535) { set_error("radial gemm: grid too large"); return E3_ERR_UNSUPPORTED; }
     static const int nprod = []() { const char *e = getenv("E3_RADIAL_PRODUCTS"); return (e && e[0] == '1') ? 1 : 3; }();
-    radial_gemm_fwd_kernel<<<dim3((unsigned)slabs, (unsigned)runs), 256, kGemmSmem, st>>>(Hhi, Hlo, W3Thi, W3Tlo, D, ldd, E, N, tiles_per_cta, nprod);
+    radial_gemm_fwd_kernel<<<dim3((unsigned)slabs, (unsigned)runs), 288, kGemmSmem, st>>>(Hhi, Hlo, W3Thi, W3Tlo, D, ldd, E, N, tiles_per_cta, nprod);
     E3_CUDA_TRY(cudaGetLastError());
     return E3_OK;
 }

@@ -160,3 +160,41 @@ def test_static_cp_async_wait_counts_equal_a_full_drain(tune, C, storage, monkey
     for r in res[0] + res[1]:
         for k in res[0][0]:
             assert np.array_equal(r[k], res[0][0][k]), (tune, k)
+
+
+def test_whole_step_is_capturable_in_a_cuda_graph():
+    """VERDICT r1 item 6 (repeated-MD-step case): every launch of a2..a7 goes to the caller's stream and nothing synchronises (validate = 0),
+    so the step captures into ONE CUDA graph; replays are bit-identical to the eager step and follow new inputs written into the same buffers."""
+    cfg = W.CONFIGS[1]
+    pl, g, x, w, G = make_case(cfg)
+    plan = gpu_plan(pl)
+    snd, rcv, vec = to_dev(g.senders), to_dev(g.receivers), to_dev(g.vec)
+    xd, wd, Gd = to_dev(x), to_dev(w), to_dev(G)
+
+    def step():
+        row_ptr, perm_s, col_ptr = B.e3_graph_prepare(snd, rcv, g.n_nodes)
+        sh = B.e3_sh_fwd(plan, vec)
+        out = B.e3_tp_scatter_fwd(plan, xd, sh, wd, snd, rcv, row_ptr, g.n_nodes)
+        dx, dY, dw = B.e3_tp_scatter_bwd(plan, xd, sh, wd, snd, rcv, row_ptr, perm_s, col_ptr, g.n_nodes, Gd)
+        dvec = B.e3_sh_bwd(plan, vec, dY)
+        return out, dx, dw, B.e3_force_reduce(dvec, row_ptr, perm_s, col_ptr, g.n_nodes)
+
+    eager = [t.clone() for t in step()]
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        step()                                                   # warm-up on the capture stream
+    torch.cuda.current_stream().wait_stream(side)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        outs = step()
+    for _ in range(3):
+        graph.replay()
+    torch.cuda.synchronize()
+    assert all(torch.equal(a, b) for a, b in zip(eager, outs))
+    xd.mul_(-0.5)                                                # new inputs in the captured buffers: the replay must follow them
+    graph.replay()
+    torch.cuda.synchronize()
+    ref = run_oracle(pl, g, -0.5 * x, w, G)
+    assert relerr(outs[0].cpu().numpy(), ref["out"]) <= TOL_FWD and relerr(outs[3].cpu().numpy(), ref["F"]) <= TOL_VJP
