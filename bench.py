@@ -508,6 +508,56 @@ def measure_config(k, args, world, rank, local, dev, steps, want_cpu, want_e2e):
         net.destroy()
         del rws
 
+    # NEXT-4 beside the headline, same graph: (i) the neighbour list built on the device from the positions,
+    # (ii) the tensor product + VJP of a plan with the paper's NequIP multiplicities (L484-L485: 64x0e+64x0o+32x1o+32x1e+32x2e+32x2o, l_max 2),
+    # which runs one generated kernel pair per multiplicity class.  Timed alone, CUDA events; reported, not part of `value`.
+    if rank == 0 and args.radial and cfg.geometry == "periodic" and cfg.storage == "f32":
+        def timed(fn, n):
+            for _ in range(2):
+                fn()
+            a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a_.record(stream)
+            for _ in range(n):
+                fn()
+            b_.record(stream)
+            torch.cuda.synchronize()
+            return a_.elapsed_time(b_) / n
+        nrep = max(3, min(steps, 20))
+        pos32 = torch.from_numpy(g.pos.astype(np.float32)).to(dev)
+        nb = B.e3_neighbor_build(pos32, (cfg.box,) * 3, W.CUTOFF, max_edges=E + 64)
+        nb_ms = timed(lambda: B.e3_neighbor_build(pos32, (cfg.box,) * 3, W.CUTOFF, max_edges=E + 64), nrep)
+        nq_in = [(0, 1, 64), (0, -1, 64), (1, -1, 32), (1, 1, 32), (2, 1, 32), (2, -1, 32)]
+        nq_out, nq_paths = B.e3_all_paths(nq_in, 2, 2)
+        nq = B.e3_plan_create(nq_in, 2, nq_out, nq_paths, B.E3_F32)
+        gq = torch.Generator(device=dev); gq.manual_seed(cfg.seed + 4000)
+        xq = torch.randn((N, nq.feats_per_node), generator=gq, device=dev)
+        Gq = torch.randn((N, nq.out_per_node), generator=gq, device=dev)
+        nwq = E * nq.weights_per_edge
+        wq = (w.view(-1)[:nwq] if w.numel() >= nwq else torch.randn(nwq, generator=gq, device=dev)).view(E, nq.weights_per_edge)   # a dense prefix of the resident weights
+        shq = B.e3_sh_fwd(nq, vec)
+        outq = torch.empty((N, nq.out_per_node), device=dev)
+        dxq = torch.empty((N, nq.feats_per_node), device=dev)
+        dwq = (gw.view(-1)[:nwq] if gw.numel() >= nwq else torch.empty(nwq, device=dev)).view(E, nq.weights_per_edge)
+        gshq = torch.empty((E, nq.sh_dim), device=dev)
+        wsq = torch.empty(B.e3_bwd_workspace_bytes(nq, E, N), dtype=torch.uint8, device=dev)
+        fq = timed(lambda: B.e3_tp_scatter_fwd(nq, xq, shq, wq, snd, rcv, row_ptr, N, out=outq), nrep)
+        bq = timed(lambda: B.e3_tp_scatter_bwd(nq, xq, shq, wq, snd, rcv, row_ptr, perm_s, col_ptr, N, Gq, grad_feats=dxq, grad_sh=gshq,
+                                               grad_weights=dwq, workspace=wsq), nrep)
+        fF, bF = nq.work()
+        wpe, fpn, opn = nq.weights_per_edge, nq.feats_per_node, nq.out_per_node
+        fB = E * (wpe * 4 + 9 * 4 + 4) + (N + 1) * 4 + N * (fpn + opn) * 4
+        bB = E * (2 * wpe * 4 + 9 * 8 + 12) + 2 * (N + 1) * 4 + N * (2 * fpn + opn) * 4
+        t_rq = max(fB / (hbm_peak * 1e9), fF * E / (FP32_PEAK_TFLOPS * 1e12)) + max(bB / (hbm_peak * 1e9), bF * E / (FP32_PEAK_TFLOPS * 1e12))
+        block["next_rows"] = {
+            "neighbor_build": {"ms": nb_ms, "edges": int(nb[0].numel()), "edges_per_s": nb[0].numel() / (nb_ms * 1e-3),
+                               "what": "e3_neighbor_build: fp32 positions -> receiver-sorted senders / receivers / vec / row_ptr (cell list, reading N1)"},
+            "nequip_multiplicities": {"irreps_in": "64x0e+64x0o+32x1o+32x1e+32x2e+32x2o", "sh_lmax": 2, "paths": len(nq_paths), "weights_per_edge": wpe,
+                                      "ms_fwd": fq, "ms_bwd": bq, "edges_per_s_fwd_plus_vjp": E / ((fq + bq) * 1e-3), "frac_of_roofline": t_rq / ((fq + bq) * 1e-3),
+                                      "algorithmic_bytes_fwd": fB, "algorithmic_bytes_bwd": bB, "kernel_info": {"fwd": nq.kernel_info(0), "bwd": nq.kernel_info(1)},
+                                      "what": "one generated kernel pair per multiplicity class (64, 32) over the rows of the whole plan; weights = a prefix of the resident weight buffer"}}
+        nq.destroy()
+        del pos32, nb, xq, Gq, shq, outq, dxq, gshq, wsq, wq, dwq
+
     # free the device-resident run before the host-buffer one (config 4 holds ~125 GB)
     del out, sh, gfe, gsh, gw, gvec, F, ws, gws, row_ptr, col_ptr, perm_s
     gc.collect()
@@ -590,7 +640,7 @@ def run_ours(args):
                 "ms_per_step": blk["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": blk["dtype"], "data": "synthetic"}
         for key in ("config", "clocks", "gpu_launches", "e2e", "roofline", "roofline_fwd", "tp_fwd_plus_vjp", "alu_peak", "kernel_ms",
-                    "kernel_info", "cpu_baseline", "radial"):
+                    "kernel_info", "cpu_baseline", "radial", "next_rows"):
             line[key] = blk.get(key)
         line["csrc_sha"] = kernel_sources_sha()
         if sec is not None:
