@@ -133,3 +133,20 @@ def test_session_host_path_with_unequal_multiplicities():
     assert relerr(hout.numpy(), ref_out) <= TOL_FWD
     assert relerr(hdx.numpy(), dx) <= TOL_VJP and relerr(hdw.numpy(), dw) <= TOL_VJP
     assert relerr(hF.numpy(), F) <= TOL_VJP
+
+
+def test_nequip_multiplicities_on_the_config2_graph():
+    """The paper's NequIP irreps (L484-L485) on a benchmark-size graph (1536 atoms, 80 518 edges, several CTA waves and both
+    multiplicity classes in the launch shapes the heuristics pick for it), whole tensors against the oracle."""
+    g, _ = W.make_graph(W.CONFIGS[2])
+    rng = np.random.default_rng(12)
+    irreps_out, paths = O.all_paths(NEQUIP, 2, 2)
+    pl = (NEQUIP, 2, irreps_out, paths)
+    in_size, sh_dim, out_size, w_size = O.tp_mul_dims(*pl)
+    n, e = g.n_nodes, g.n_edges
+    x = rng.normal(size=(n, in_size)).astype(np.float32)
+    w = (rng.normal(size=(e, w_size)) / np.sqrt(len(paths))).astype(np.float32)
+    G = rng.normal(size=(n, out_size)).astype(np.float32)
+    _, errs = _run_both(pl, (in_size, sh_dim, out_size, w_size), g.senders, g.receivers, g.vec, x, w, G)
+    print({k: f"{v:.2e}" for k, v in errs.items()})
+    assert errs["out"] <= TOL_FWD and max(errs["dx"], errs["dY"], errs["dw"]) <= TOL_VJP, errs
