@@ -452,33 +452,37 @@ __global__ void __launch_bounds__(288, 1) radial_gemm_fwd_kernel(const float *__
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 256;" :: "r"(tmem) : "memory");
 }
 
-// BACKWARD: D[256-row tile, 64] = sum over K chunks of 32 of A[256 x Kt] * B[64 x Kt]^T (A = grad_weights, fp32, streamed from HBM;
-// B = W3 as TF32 high / low parts).  A CTA owns TWO 128-row MMA tiles (two TMEM accumulators of 64 columns) that share every B chunk:
-// each 256-row tile re-reads all of W3 (hi + lo, 1.1 MB on config 4) instead of each 128-row tile -- the first version's W3 traffic
-// equalled its grad_weights traffic (45.5 GB each) and its time was set by the operand copies, not by the MMAs (radial GEMM
-// experiments).  Chunks of K = 32 keep the register staging (chunks kc + 1, kc + 2 in flight in registers while chunk kc is multiplied)
-// and the two 80 KB shared-memory stages the same size as before.  Canonical K-major no-swizzle layout with 32-wide rows: core matrices
-// of 8 rows x 16 bytes, 128 bytes apart along K (LBO), groups of 8 rows 1024 bytes apart (SBO).
-__device__ __forceinline__ uint64_t umma_desc32(uint32_t smem_addr)
+// BACKWARD: D[128 NT-row tile, 64] = sum over K chunks of 64 / NT of A[rows x Kt] * B[64 x Kt]^T (A = grad_weights, fp32, streamed from
+// HBM; B = W3 as TF32 high / low parts).  A CTA owns NT = 2 or 4 128-row MMA tiles (NT TMEM accumulators of 64 columns) that share every
+// B chunk: each 256- or 512-row tile re-reads all of W3 (hi + lo, 1.1 MB on config 4) instead of each 128-row tile -- the first
+// version's W3 traffic equalled its grad_weights traffic (45.5 GB each) and its time was set by the operand copies and the per-chunk
+// synchronisation, not by the MMAs (radial GEMM experiments).  Chunks of K = 64 / NT keep the register staging (chunks
+// kc + 1, kc + 2 in flight in registers while chunk kc is multiplied) and the shared-memory stages the size they were.  Canonical
+// K-major no-swizzle layout with K-wide rows: core matrices of 8 rows x 16 bytes, 128 bytes apart along K (LBO), groups of 8 rows
+// 32 K bytes apart (SBO).
+template <int SBO>
+__device__ __forceinline__ uint64_t umma_desc_sbo(uint32_t smem_addr)
 {
     uint64_t d = 0;
     d |= (uint64_t)((smem_addr >> 4) & 0x3fff);
     d |= (uint64_t)((128u >> 4) & 0x3fff) << 16;
-    d |= (uint64_t)((1024u >> 4) & 0x3fff) << 32;
+    d |= (uint64_t)(((uint32_t)SBO >> 4) & 0x3fff) << 32;
     d |= (uint64_t)1 << 46;
     return d;
 }
-__device__ __forceinline__ uint32_t canon_off32(int row, int k)  // byte offset of element (row, k) of a [rows x 32] fp32 tile
+template <int SBO>
+__device__ __forceinline__ uint32_t canon_off_sbo(int row, int k)  // byte offset of element (row, k) of a [rows x SBO/32] fp32 tile
 {
-    return (uint32_t)((row >> 3) * 1024 + (k >> 2) * 128 + (row & 7) * 16 + (k & 3) * 4);
+    return (uint32_t)((row >> 3) * SBO + (k >> 2) * 128 + (row & 7) * 16 + (k & 3) * 4);
 }
-// the three products of one 32-wide K chunk (4 MMA steps of K = 8) of one 128-row tile: lo*hi, hi*lo, hi*hi
-__device__ __forceinline__ void issue_chunk32(uint32_t tmem_d, uint32_t sAhi, uint32_t sAlo, uint32_t sBhi, uint32_t sBlo, uint32_t idesc, bool first)
+// the three products of one K chunk (KS MMA steps of K = 8) of one 128-row tile: lo*hi, hi*lo, hi*hi
+template <int KS, int SBO>
+__device__ __forceinline__ void issue_chunk_t(uint32_t tmem_d, uint32_t sAhi, uint32_t sAlo, uint32_t sBhi, uint32_t sBlo, uint32_t idesc, bool first)
 {
 #pragma unroll
-    for (int ks = 0; ks < 4; ++ks) {
-        const uint64_t ahi = umma_desc32(sAhi + ks * 256), alo = umma_desc32(sAlo + ks * 256);
-        const uint64_t bhi = umma_desc32(sBhi + ks * 256), blo = umma_desc32(sBlo + ks * 256);
+    for (int ks = 0; ks < KS; ++ks) {
+        const uint64_t ahi = umma_desc_sbo<SBO>(sAhi + ks * 256), alo = umma_desc_sbo<SBO>(sAlo + ks * 256);
+        const uint64_t bhi = umma_desc_sbo<SBO>(sBhi + ks * 256), blo = umma_desc_sbo<SBO>(sBlo + ks * 256);
         const uint32_t acc0 = (!first || ks > 0) ? 1u : 0u;
         asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}"
                      :: "r"(tmem_d), "l"(alo), "l"(bhi), "r"(idesc), "r"(acc0) : "memory");
@@ -489,11 +493,18 @@ __device__ __forceinline__ void issue_chunk32(uint32_t tmem_d, uint32_t sAhi, ui
     }
 }
 
-constexpr int kBwdRows = 256, kBwdK = 32, kBwdStage = 81920;      // stage: A hi 32 KB | A lo 32 KB | B hi 8 KB | B lo 8 KB
-
+// kBwdTiles 128-row MMA tiles per CTA (template parameter NT: 4 for large edge counts, 2 when 512-row CTAs would leave the machine
+// with too few waves); rows x K chunk = 8192 elements per stage whatever the split
+template <int NT>
 __global__ void __launch_bounds__(256, 1) radial_gemm_bwd_kernel(const float *__restrict__ A, long long lda, const float *__restrict__ Bhi,
                                                                  const float *__restrict__ Blo, long long ldb, float *__restrict__ D, long long M, long long Kt)
 {
+    constexpr int kBwdTiles = NT;
+    constexpr int kBwdRows = 128 * kBwdTiles, kBwdK = 64 / kBwdTiles;
+    constexpr int kBwdQPR = kBwdK / 4, kBwdPP = kBwdQPR / 4;           // 16-byte quads per row; passes per 64-row block
+    constexpr int kBwdSBO = kBwdQPR * 128;                             // bytes between groups of 8 rows
+    constexpr int kBwdB = 64 * kBwdK * 4;                              // one B plane
+    constexpr int kBwdStage = 65536 + 2 * kBwdB;                       // stage: A hi 32 KB | A lo 32 KB | B hi | B lo
     extern __shared__ __align__(1024) unsigned char smem[];
     __shared__ __align__(8) unsigned long long mbar[2];
     __shared__ uint32_t tmem_base_s;
@@ -501,7 +512,7 @@ __global__ void __launch_bounds__(256, 1) radial_gemm_bwd_kernel(const float *__
     const long long m0 = (long long)blockIdx.x * kBwdRows;
     const uint32_t mbar_s = (uint32_t)__cvta_generic_to_shared(&mbar[0]);
     if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 128;" :: "r"((uint32_t)__cvta_generic_to_shared(&tmem_base_s)) : "memory");
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"((uint32_t)__cvta_generic_to_shared(&tmem_base_s)), "n"(64 * kBwdTiles) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     if (tid == 0) {
@@ -516,22 +527,21 @@ __global__ void __launch_bounds__(256, 1) radial_gemm_bwd_kernel(const float *__
     const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(kH >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
     const uint32_t smem_s = (uint32_t)__cvta_generic_to_shared(smem);
     const int k_chunks = (int)((Kt + kBwdK - 1) / kBwdK);
-    const bool second = m0 + kTileM < M;                 // the second 128-row tile holds rows
     // thread -> pieces of a chunk: A [256 x 8 quads]: pass j: row = (j / 2) * 64 + 8 warp + (lane & 7), quad = (j & 1) * 4 + (lane >> 3);
     // B [64 x 8 quads]: pass j: row = 8 warp + (lane & 7), quad = 4 j + (lane >> 3).  A warp covers 8 rows x 64 bytes: whole sectors in global
     // memory, 512 contiguous bytes in the canonical layout (conflict-free).
     const int r8 = warp * 8 + (lane & 7), q4 = lane >> 3;
-    float4 ra0[8], rbh0[2], rbl0[2], ra1[8], rbh1[2], rbl1[2];
-    auto load_chunk = [&](int kc, float4 (&ra)[8], float4 (&rbh)[2], float4 (&rbl)[2]) {
+    float4 ra0[8], rbh0[kBwdPP], rbl0[kBwdPP], ra1[8], rbh1[kBwdPP], rbl1[kBwdPP];
+    auto load_chunk = [&](int kc, float4 (&ra)[8], float4 (&rbh)[kBwdPP], float4 (&rbl)[kBwdPP]) {
         const long long k0 = (long long)kc * kBwdK;
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
-            const int row = (j >> 1) * 64 + r8, q = (j & 1) * 4 + q4;
+            const int row = (j / kBwdPP) * 64 + r8, q = (j % kBwdPP) * 4 + q4;
             ra[j] = make_float4(0.f, 0.f, 0.f, 0.f);
             if (m0 + row < M && k0 + q * 4 + 4 <= Kt) ra[j] = __ldcs(reinterpret_cast<const float4 *>(A + (m0 + row) * lda + k0 + q * 4));
         }
 #pragma unroll
-        for (int j = 0; j < 2; ++j) {
+        for (int j = 0; j < kBwdPP; ++j) {
             const int q = j * 4 + q4;
             rbh[j] = make_float4(0.f, 0.f, 0.f, 0.f); rbl[j] = rbh[j];
             if (k0 + q * 4 + 4 <= Kt) {
@@ -540,26 +550,26 @@ __global__ void __launch_bounds__(256, 1) radial_gemm_bwd_kernel(const float *__
             }
         }
     };
-    auto store_chunk = [&](int buf, const float4 (&ra)[8], const float4 (&rbh)[2], const float4 (&rbl)[2]) {
+    auto store_chunk = [&](int buf, const float4 (&ra)[8], const float4 (&rbh)[kBwdPP], const float4 (&rbl)[kBwdPP]) {
         unsigned char *base = smem + buf * kBwdStage;
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
-            const int row = (j >> 1) * 64 + r8, q = (j & 1) * 4 + q4;
+            const int row = (j / kBwdPP) * 64 + r8, q = (j % kBwdPP) * 4 + q4;
             const float4 v = ra[j];
             const float4 h = make_float4(tf32_hi(v.x), tf32_hi(v.y), tf32_hi(v.z), tf32_hi(v.w));
-            const uint32_t off = canon_off32(row, q * 4);
+            const uint32_t off = canon_off_sbo<kBwdSBO>(row, q * 4);
             *reinterpret_cast<float4 *>(base + off) = h;
             *reinterpret_cast<float4 *>(base + 32768 + off) = make_float4(v.x - h.x, v.y - h.y, v.z - h.z, v.w - h.w);
         }
 #pragma unroll
-        for (int j = 0; j < 2; ++j) {
-            const uint32_t off = canon_off32(r8, (j * 4 + q4) * 4);
+        for (int j = 0; j < kBwdPP; ++j) {
+            const uint32_t off = canon_off_sbo<kBwdSBO>(r8, (j * 4 + q4) * 4);
             *reinterpret_cast<float4 *>(base + 65536 + off) = rbh[j];
-            *reinterpret_cast<float4 *>(base + 73728 + off) = rbl[j];
+            *reinterpret_cast<float4 *>(base + 65536 + kBwdB + off) = rbl[j];
         }
     };
     uint32_t ph0 = 0, ph1 = 0;
-    auto step = [&](int kc, int buf, float4 (&ra)[8], float4 (&rbh)[2], float4 (&rbl)[2], uint32_t &ph) {
+    auto step = [&](int kc, int buf, float4 (&ra)[8], float4 (&rbh)[kBwdPP], float4 (&rbl)[kBwdPP], uint32_t &ph) {
         if (kc >= 2) {                                   // the MMAs of chunk kc - 2 must have finished reading this stage
             mbar_wait_parity(mbar_s + buf * 8, ph);
             ph ^= 1u;
@@ -572,8 +582,10 @@ __global__ void __launch_bounds__(256, 1) radial_gemm_bwd_kernel(const float *__
         if (tid == 0) {
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             const uint32_t b = smem_s + buf * kBwdStage;
-            issue_chunk32(tmem, b, b + 32768, b + 65536, b + 73728, idesc, kc == 0);
-            if (second) issue_chunk32(tmem + 64, b + 16384, b + 32768 + 16384, b + 65536, b + 73728, idesc, kc == 0);
+#pragma unroll
+            for (int t = 0; t < kBwdTiles; ++t)          // tile t: rows 128 t .. 128 t + 127 of the stage, accumulator columns 64 t ..
+                if (t == 0 || m0 + t * kTileM < M)
+                    issue_chunk_t<kBwdK / 8, kBwdSBO>(tmem + 64 * t, b + t * 16 * kBwdSBO, b + 32768 + t * 16 * kBwdSBO, b + 65536, b + 65536 + kBwdB, idesc, kc == 0);
             asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(mbar_s + buf * 8) : "memory");
         }
     };
@@ -588,12 +600,12 @@ __global__ void __launch_bounds__(256, 1) radial_gemm_bwd_kernel(const float *__
         mbar_wait_parity(mbar_s + buf * 8, buf ? ph1 : ph0);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         float *stg = reinterpret_cast<float *>(smem + ((k_chunks & 1) ? kBwdStage : 0));       // the stage the last chunk did not use
-        epilogue_tile<kH>(tmem, warp, lane, stg, D, kH, m0, M, 0, kH);
-        if (second) epilogue_tile<kH>(tmem + 64, warp, lane, stg, D, kH, m0 + kTileM, M, 0, kH);
+        for (int t = 0; t < kBwdTiles; ++t)
+            if (t == 0 || m0 + t * kTileM < M) epilogue_tile<kH>(tmem + 64 * t, warp, lane, stg, D, kH, m0 + t * kTileM, M, 0, kH);
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
-    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 128;" :: "r"(tmem) : "memory");
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem), "n"(64 * kBwdTiles) : "memory");
 }
 
 constexpr int kGemmSmem = 196608;      // forward: 2 x 64 KB of A + 64 KB of B; backward: 2 x 96 KB stages (the epilogue stages through an idle buffer)
@@ -603,7 +615,8 @@ int launch_gemm_fwd(const float *Hhi, const float *Hlo, const float *W3Thi, cons
     static bool attr_set = false;
     if (!attr_set) {
         E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
-        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
+        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
+        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
         attr_set = true;
     }
     if (E <= 0) return E3_OK;
@@ -627,13 +640,17 @@ int launch_gemm_bwd(const float *A, long long lda, const float *Bhi, const float
     static bool attr_set = false;
     if (!attr_set) {
         E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
-        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
+        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
+        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
         attr_set = true;
     }
     if (M <= 0) return E3_OK;
-    const long long grid = (M + kBwdRows - 1) / kBwdRows;
+    // 512-row CTAs once they still give the machine four waves (every CTA re-reads all of W3), 256-row CTAs below that
+    const int nt = M >= 4LL * 148 * 512 ? 4 : 2;
+    const long long grid = (M + 128 * nt - 1) / (128 * nt);
     if (grid > 0x7fffffffLL) { set_error("radial gemm: grid too large"); return E3_ERR_UNSUPPORTED; }
-    radial_gemm_bwd_kernel<<<(unsigned)grid, 256, kGemmSmem, st>>>(A, lda, Bhi, Blo, ldb, D, M, Kt);
+    if (nt == 4) radial_gemm_bwd_kernel<4><<<(unsigned)grid, 256, kGemmSmem, st>>>(A, lda, Bhi, Blo, ldb, D, M, Kt);
+    else radial_gemm_bwd_kernel<2><<<(unsigned)grid, 256, kGemmSmem, st>>>(A, lda, Bhi, Blo, ldb, D, M, Kt);
     E3_CUDA_TRY(cudaGetLastError());
     return E3_OK;
 }
