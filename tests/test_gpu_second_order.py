@@ -128,3 +128,33 @@ def test_hessian_row_config1_against_oracle():
     errs = dict(row=relerr(row.cpu().numpy(), rrow), gx=relerr(so["gx"].cpu().numpy(), rgx), gw=relerr(so["gw"].cpu().numpy(), rgw))
     print({k: f"{v:.1e}" for k, v in errs.items()})
     assert max(errs.values()) <= 2 * TOL_VJP, errs
+
+
+def test_vjp_vjp_with_unequal_multiplicities():
+    """NEXT-2 on a NEXT-4 plan: the second-order call goes through the same launch helpers, so a plan with the paper's NequIP multiplicity
+    pattern (L484-L485; one kernel pair per multiplicity class) must match the general-multiplicity oracle as well."""
+    rng = np.random.default_rng(21)
+    irreps_in = [(0, 1, 64), (0, -1, 64), (1, -1, 32), (1, 1, 32), (2, 1, 32), (2, -1, 32)]
+    irreps_out, paths = O.all_paths(irreps_in, 2, 2)
+    pl = (irreps_in, 2, irreps_out, paths)
+    in_size, sh_dim, out_size, w_size = O.tp_mul_dims(*pl)
+    n = 17
+    deg = rng.integers(0, 9, size=n); deg[3] = 0
+    rcv = np.repeat(np.arange(n), deg)
+    snd = rng.integers(0, n, size=rcv.size)
+    o = np.lexsort((snd, rcv))
+    snd, rcv = snd[o].astype(np.int32), rcv[o].astype(np.int32)
+    e = rcv.size
+    f32 = lambda a: a.astype(np.float32)
+    t = dict(x=f32(rng.normal(size=(n, in_size))), Y=f32(rng.normal(size=(e, sh_dim))), w=f32(rng.normal(size=(e, w_size))),
+             g=f32(rng.normal(size=(n, out_size))), vx=f32(rng.normal(size=(n, in_size))), vY=f32(rng.normal(size=(e, sh_dim))),
+             vw=f32(rng.normal(size=(e, w_size))))
+    plan = B.e3_plan_create(*pl)
+    sd, rd = to_dev(snd), to_dev(rcv)
+    rp, ps, cp = B.e3_graph_prepare(sd, rd, n)
+    d = {k: to_dev(v) for k, v in t.items()}
+    got = B.e3_tp_scatter_vjp_vjp(plan, d["x"], d["Y"], d["w"], sd, rd, rp, ps, cp, n, d["g"], d["vx"], d["vY"], d["vw"])
+    ref = dict(zip(("gg", "gx", "gY", "gw"), O.tp_vjp_vjp(*pl, t["x"], t["Y"], t["w"], snd, rcv, n, t["g"], t["vx"], t["vY"], t["vw"])))
+    torch.cuda.synchronize()
+    errs = {k: relerr(got[k].cpu().numpy(), ref[k]) for k in ref}
+    assert max(errs.values()) <= TOL_VJP, errs

@@ -135,6 +135,39 @@ def test_vjp_vjp_against_finite_differences_of_the_first_order_oracle():
     assert abs((a * vY).sum() - (b * vx).sum()) < 1e-11
 
 
+def test_vjp_vjp_with_unequal_multiplicities_is_the_composition_of_pinned_calls():
+    """orc_tp_vjp_vjp on a plan with per-irrep multiplicities (NEXT-2 x NEXT-4) against the composition identities built from the pinned
+    general-multiplicity first-order oracle (orc_tp_mul_*) and against central differences of it."""
+    rng = np.random.default_rng(31)
+    irreps_in, irreps_out, paths = _nequip_like()
+    pl = (irreps_in, 2, irreps_out, paths)
+    in_size, sh_dim, out_size, w_size = O.tp_mul_dims(*pl)
+    n, e = 5, 13
+    snd, rcv = _graph(rng, n, e)
+    x = rng.normal(size=(n, in_size)); Y = rng.normal(size=(e, sh_dim)); w = rng.normal(size=(e, w_size)); g = rng.normal(size=(n, out_size))
+    vx = rng.normal(size=x.shape); vY = rng.normal(size=Y.shape); vw = rng.normal(size=w.shape)
+    gg, gx, gY, gw = O.tp_vjp_vjp(*pl, x, Y, w, snd, rcv, n, g, vx, vY, vw)
+    T = lambda a, b, c: O.tp_mul_fwd(*pl, a, b, c, snd, rcv, n)
+    D = lambda a, b, c: O.tp_mul_bwd(*pl, a, b, c, snd, rcv, n, g)
+    assert np.abs(gg - (T(vx, Y, w) + T(x, vY, w) + T(x, Y, vw))).max() < 1e-12
+    assert np.abs(gx - (D(x, vY, w)[0] + D(x, Y, vw)[0])).max() < 1e-12
+    assert np.abs(gY - (D(vx, Y, w)[1] + D(x, Y, vw)[1])).max() < 1e-12
+    assert np.abs(gw - (D(vx, Y, w)[2] + D(x, vY, w)[2])).max() < 1e-12
+
+    def S(x_, Y_, w_):
+        dx, dY, dw = O.tp_mul_bwd(*pl, x_, Y_, w_, snd, rcv, n, g)
+        return float((vx * dx).sum() + (vY * dY).sum() + (vw * dw).sum())
+    h = 1e-6
+    for k, (arr, grad) in enumerate(((x, gx), (Y, gY), (w, gw))):
+        for _ in range(8):
+            idx = tuple(rng.integers(0, s_) for s_ in arr.shape)
+            ap, am = arr.copy(), arr.copy(); ap[idx] += h; am[idx] -= h
+            args_p, args_m = [x, Y, w], [x, Y, w]
+            args_p[k], args_m[k] = ap, am
+            fd = (S(*args_p) - S(*args_m)) / (2 * h)
+            assert abs(fd - grad[idx]) < 2e-7 * max(1.0, abs(fd))
+
+
 @pytest.mark.parametrize("lmax", [1, 2, 3])
 def test_sh_second_derivative(lmax):
     rng = np.random.default_rng(10 + lmax)
