@@ -65,6 +65,7 @@ def main():
     for i, m in enumerate(hdr):
         if "issue_stalled" in m and m.endswith("per_issue_active.ratio") and "not_issued" not in m:
             vals = [float(r[i] or 0) for r in data]
+            vals = [0.0 if v != v else v for v in vals]
             if max(vals) > 0.05:
                 lines.append(f"| `{m}` | inst | " + " | ".join(f"{v:.2f}" for v in vals) + " |")
     out_md = os.path.join(ROOT, "profiles", a.name + ".md")
@@ -76,6 +77,9 @@ def main():
     ent = traffic.setdefault(a.workload, {})
     for r, n in zip(data, names):
         b = float(r[ir]) * UNIT_SCALE[units[ir]] + float(r[iw]) * UNIT_SCALE[units[iw]]
+        if b != b:             # ncu could not collect this launch's memory counters (NaN in the report): no entry, bench.py reports null
+            ent.pop(n, None)
+            continue
         ent[n] = {"dram_bytes": int(b), "dram_read_bytes": int(float(r[ir]) * UNIT_SCALE[units[ir]]),
                   "dram_write_bytes": int(float(r[iw]) * UNIT_SCALE[units[iw]]), "duration": f"{r[it]} {units[it]}",
                   "capture": f"profiles/{a.name}.md", "csrc_sha": sha,
