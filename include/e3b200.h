@@ -161,6 +161,11 @@ int e3_tp_scatter_fwd(const e3_plan *plan, const void *feats /*[N,in_dim*C]*/, c
  * dtype and may be NULL (skipped).  workspace: >= e3_bwd_workspace_bytes(plan, E, N) bytes; it
  * holds the per-edge grad_feats contributions that the second phase sums per sender in
  * ascending edge order (deterministic, no atomics).
+ * Opt-in (E3_TUNE bwd_overlap=K at plan creation, `receivers` given): the first phase is launched in K receiver chunks on `stream` and
+ * the sums of the senders each chunk completes run meanwhile on a stream owned by the plan; that stream waits for everything enqueued on
+ * `stream` before the call and `stream` waits for it before the call returns, so the call behaves like a single-stream one (it can be
+ * captured in a CUDA graph) and its results are bit-identical to the default path.  Measured slower on power-capped boards,
+ * hence off by default.  `receivers` may be NULL.  One VJP call of a plan at a time when the overlap is on.
  * -------------------------------------------------------------------------------------------*/
 size_t e3_bwd_workspace_bytes(const e3_plan *plan, int64_t n_edges, int32_t n_nodes);
 int e3_tp_scatter_bwd(const e3_plan *plan, const void *feats, const void *sh, const void *weights,

@@ -102,6 +102,12 @@ struct e3_plan {
     int n_sm = 148;            // SM count of the device the plan was created on
     e3::JitKernel fwd, bwd;
     cudaEvent_t mid_event = nullptr;   // profiling aid, see e3_profile_set_mid_event
+    // VJP overlap: the first phase is launched in `bwd_overlap` receiver chunks and the per-sender reduction of the
+    // senders a chunk completes runs on a side stream while the next chunk computes.  -1 / 0 = off (the default: measured slower), K = K chunks.
+    int bwd_overlap = -1;
+    static constexpr int kMaxOverlap = 16;
+    cudaStream_t side_stream = nullptr;
+    cudaEvent_t ov_ev[kMaxOverlap + 1] = {};
 
     // Element layout of a node row / a weights row.  A regular plan (all multiplicities equal to C) has its irrep blocks back to
     // back, (2l+1)*C elements each.  NEXT-4, unequal multiplicities: the plan is a COMPOSITE of one sub-plan per multiplicity
@@ -170,7 +176,7 @@ int launch_graph_prepare(const int32_t *snd, const int32_t *rcv, int64_t E, int3
 int launch_force_reduce(const float *gvec, const int32_t *row_ptr, const int32_t *perm_s, const int32_t *col_ptr,
                         int64_t E, int32_t N, float *forces, cudaStream_t st);
 int launch_dx_reduce(const float *dxe, const int32_t *perm_s, const int32_t *col_ptr, int32_t N, int row_len,
-                     float *dx, cudaStream_t st);
+                     float *dx, cudaStream_t st, const int32_t *receivers = nullptr, int32_t r_lo = 0, int32_t r_hi = 0);
 int launch_gsh_reduce(const float *parts, int n_parts, int64_t n, float *gsh, cudaStream_t st);
 int measure_fp32_peak(double *tflops, double ms_target, cudaStream_t st);
 int launch_sh_bwd_bwd(int lmax, const float *vec, const float *gsh, const float *u, int64_t E, float *g_vec, float *g_sh, cudaStream_t st);

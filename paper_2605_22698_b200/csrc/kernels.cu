@@ -464,12 +464,21 @@ int launch_force_reduce(const float *gvec, const int32_t *row_ptr, const int32_t
 // ---------------------------------------------------------------------------------------------
 template <int VEC>
 __global__ void dx_reduce_kernel(const float *__restrict__ dxe, const int32_t *__restrict__ perm_s,
-                                 const int32_t *__restrict__ col_ptr, int row_len, float *__restrict__ dx)
+                                 const int32_t *__restrict__ col_ptr, int row_len, float *__restrict__ dx,
+                                 const int32_t *__restrict__ receivers, int32_t r_lo, int32_t r_hi)
 {
     constexpr int TILE = 512, U = 8;            // edge ids staged per pass; rows in flight per thread
     __shared__ int32_t eid[TILE];
     const int32_t s = blockIdx.x;
     const int32_t a = col_ptr[s], b = col_ptr[s + 1];
+    if (receivers) {
+        // ranged call (the VJP overlaps this reduction with the first phase, receiver chunk by receiver chunk): only the senders whose
+        // LAST out-edge -- the largest edge id, hence the largest receiver -- falls into [r_lo, r_hi) are complete now and are summed
+        // by this launch; senders without out-edges belong to the first range.  Every sender is summed by exactly one launch, in the
+        // same perm_s order as the single launch: results are bit-identical.
+        const int32_t rmax = b > a ? receivers[perm_s[b - 1]] : 0;
+        if (rmax < r_lo || rmax >= r_hi) return;
+    }
     // each thread owns up to two column groups (row_len <= 2 * blockDim.x * VEC covers every plan up to l = 3, C = 128 * 4)
     for (int c0 = 0; c0 < row_len; c0 += blockDim.x * VEC) {
         const int c = c0 + threadIdx.x * VEC;
@@ -544,16 +553,16 @@ int launch_gsh_reduce(const float *parts, int n_parts, int64_t n, float *gsh, cu
 }
 
 int launch_dx_reduce(const float *dxe, const int32_t *perm_s, const int32_t *col_ptr, int32_t N, int row_len,
-                     float *dx, cudaStream_t st)
+                     float *dx, cudaStream_t st, const int32_t *receivers, int32_t r_lo, int32_t r_hi)
 {
     if (N == 0) return E3_OK;
     if (row_len % 4 == 0) {
         int th = row_len / 4;
         th = th > 256 ? 256 : ((th + 31) / 32) * 32;
-        dx_reduce_kernel<4><<<(unsigned)N, th, 0, st>>>(dxe, perm_s, col_ptr, row_len, dx);
+        dx_reduce_kernel<4><<<(unsigned)N, th, 0, st>>>(dxe, perm_s, col_ptr, row_len, dx, receivers, r_lo, r_hi);
     } else {
         int th = row_len > 256 ? 256 : ((row_len + 31) / 32) * 32;
-        dx_reduce_kernel<1><<<(unsigned)N, th, 0, st>>>(dxe, perm_s, col_ptr, row_len, dx);
+        dx_reduce_kernel<1><<<(unsigned)N, th, 0, st>>>(dxe, perm_s, col_ptr, row_len, dx, receivers, r_lo, r_hi);
     }
     E3_CUDA_TRY(cudaGetLastError());
     return E3_OK;

@@ -468,6 +468,7 @@ void plan_make_roles(e3_plan &pl)
     tune_get("fwd_minb", pl.fwd_minb); tune_get("bwd_minb", pl.bwd_minb);
     tune_get("fwd_warps", pl.fwd_warps); tune_get("bwd_warps", pl.bwd_warps);
     tune_get("fwd_depth", pl.fwd_depth); tune_get("chunk", pl.fwd_chunk); tune_get("wait_all", pl.wait_all);
+    tune_get("bwd_overlap", pl.bwd_overlap);
     // third-generation forward: roles aligned with the input irreps, grouped into teams that share one CTA and one copy of
     // the sender rows per edge
     tune_get("fwd_v3_bulk", pl.fwd_v3_bulk);
