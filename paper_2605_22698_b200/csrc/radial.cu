@@ -327,10 +327,10 @@ __device__ __forceinline__ void epilogue_tile(uint32_t tmem_d, int warp8, int la
 // tile i + 1 are in flight; one __syncthreads and one mbarrier wait per tile.
 __global__ void __launch_bounds__(288, 1) radial_gemm_fwd_kernel(const float *__restrict__ Hhi, const float *__restrict__ Hlo, const float *__restrict__ W3Thi,
                                                                  const float *__restrict__ W3Tlo, float *__restrict__ D, long long ldd, long long E, int N,
-                                                                 int tiles_per_cta, int nprod)
+                                                                 int tiles_per_cta, int nprod, int dbg)
 {
     constexpr int NT = 64;                                                   // edges per tile (MMA N)
-    extern __shared__ __align__(1024) unsigned char smem[];                  // [slab 0 hi | slab 0 lo | slab 1 hi | slab 1 lo] 32 KB each, then 2 x [B hi | B lo] 16 KB each
+    extern __shared__ __align__(1024) unsigned char smem[];                  // [slab 0 hi | slab 0 lo | slab 1 hi | slab 1 lo] 32 KB each, then 3 x [B hi | B lo] 16 KB each
     __shared__ __align__(8) unsigned long long mbar[2];
     __shared__ uint32_t tmem_base_s;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -369,6 +369,7 @@ __global__ void __launch_bounds__(288, 1) radial_gemm_fwd_kernel(const float *__
         }
     auto issue_b = [&](long long t, int buf) {
         if (!worker) return;
+        if ((dbg & 4) || t >= t_end) { asm volatile("cp.async.commit_group;" ::: "memory"); return; }     // always one group per call
         const long long e0 = t * NT;
         const uint32_t bh = sB_s + buf * 32768, bl = bh + 16384;
 #pragma unroll
@@ -383,6 +384,7 @@ __global__ void __launch_bounds__(288, 1) radial_gemm_fwd_kernel(const float *__
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
     issue_b(t_begin, 0);
+    issue_b(t_begin + 1, 1);
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
@@ -407,7 +409,7 @@ __global__ void __launch_bounds__(288, 1) radial_gemm_fwd_kernel(const float *__
                            "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
                          : "r"(taddr) : "memory");
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-            if (feat < N) {
+            if (feat < N && !(dbg & 1)) {
                 float *dp = D + (e0 + c0) * ldd + feat;
                 if (e0 + c0 + 32 <= E) {                 // whole block inside the graph: no per-store predicate
 #pragma unroll
@@ -421,32 +423,37 @@ __global__ void __launch_bounds__(288, 1) radial_gemm_fwd_kernel(const float *__
         }
     };
     uint32_t ph0 = 0, ph1 = 0;
+    // Tile t's B operand is copied two tiles ahead into a three-deep ring and its MMAs are issued right after the tile's barrier, i.e.
+    // BEHIND the still running MMAs of tile t - 1: the tensor pipe never waits for a copy or a barrier.  The workers then wait for tile
+    // t - 1 (its B buffer is the one tile t + 2 goes to, its accumulators are what they drain next).
     for (long long t = t_begin; t < t_end; ++t) {
-        const int i = (int)(t - t_begin), buf = i & 1;
-        // B[buf ^ 1] was last read by the MMAs of tile t - 1, whose completion every thread has waited for: refill it now, so that the
-        // copies of tile t + 1 are in flight during the MMAs of tile t and the drain of tile t - 1
-        if (t + 1 < t_end) {
-            issue_b(t + 1, buf ^ 1);
-            asm volatile("cp.async.wait_group 1;" ::: "memory");             // tile t (and, the first time, the slabs) has landed
-        } else {
-            asm volatile("cp.async.wait_group 0;" ::: "memory");
-        }
+        const int i = (int)(t - t_begin), bb = i % 3, tb = i & 1;
+        asm volatile("cp.async.wait_group 1;" ::: "memory");                 // tile t (and, the first time, the slabs) has landed
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-        __syncthreads();                                                     // also: every warp has drained TMEM buffer `buf` (tile t - 2)
-        if (tid == 256) {
+        __syncthreads();                                                     // also: every warp has drained TMEM buffer `tb` (tile t - 2)
+        if (tid == 256 && !(dbg & 2)) {
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            const uint32_t bh = sB_s + buf * 32768, bl = bh + 16384;
-            issue_chunk(tmem + buf * 128, sA_s, sA_s + 32768, bh, bl, idesc, true, nprod);
-            if (two) issue_chunk(tmem + buf * 128 + 64, sA_s + 65536, sA_s + 98304, bh, bl, idesc, true, nprod);
-            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(mbar_s + buf * 8) : "memory");
+            const uint32_t bh = sB_s + bb * 32768, bl = bh + 16384;
+            issue_chunk(tmem + tb * 128, sA_s, sA_s + 32768, bh, bl, idesc, true, nprod);
+            if (two) issue_chunk(tmem + tb * 128 + 64, sA_s + 65536, sA_s + 98304, bh, bl, idesc, true, nprod);
+            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(mbar_s + tb * 8) : "memory");
         }
-        if (i > 0) epilogue(t - 1, buf ^ 1);             // overlaps the MMAs of tile t
-        mbar_wait_parity(mbar_s + buf * 8, buf ? ph1 : ph0);                 // tile t: MMAs done -> B[buf] is free, its accumulators are ready
-        if (buf) ph1 ^= 1u; else ph0 ^= 1u;
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        if (i > 0 && !(dbg & 2)) {                       // tile t - 1: MMAs done -> its B buffer is free, its accumulators are ready
+            mbar_wait_parity(mbar_s + (tb ^ 1) * 8, (tb ^ 1) ? ph1 : ph0);
+            if (tb ^ 1) ph1 ^= 1u; else ph0 ^= 1u;
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        }
+        issue_b(t + 2, (i + 2) % 3);
+        if (i > 0) epilogue(t - 1, tb ^ 1);
     }
-    epilogue(t_end - 1, (int)((t_end - 1 - t_begin) & 1));
+    {
+        const int tb = (int)((t_end - 1 - t_begin) & 1);
+        if (!(dbg & 2)) mbar_wait_parity(mbar_s + tb * 8, tb ? ph1 : ph0);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        epilogue(t_end - 1, tb);
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 256;" :: "r"(tmem) : "memory");
@@ -608,13 +615,14 @@ __global__ void __launch_bounds__(256, 1) radial_gemm_bwd_kernel(const float *__
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem), "n"(64 * kBwdTiles) : "memory");
 }
 
-constexpr int kGemmSmem = 196608;      // forward: 2 x 64 KB of A + 64 KB of B; backward: 2 x 96 KB stages (the epilogue stages through an idle buffer)
+constexpr int kGemmSmemFwd = 229376;   // forward: 2 x 64 KB of A + 3 x 32 KB of B
+constexpr int kGemmSmem = 196608;      //; backward: 2 x 96 KB stages (the epilogue stages through an idle buffer)
 
 int launch_gemm_fwd(const float *Hhi, const float *Hlo, const float *W3Thi, const float *W3Tlo, float *D, long long ldd, long long E, int N, cudaStream_t st)
 {
     static bool attr_set = false;
     if (!attr_set) {
-        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
+        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmemFwd));
         E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
         E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
         attr_set = true;
@@ -630,7 +638,8 @@ int launch_gemm_fwd(const float *Hhi, const float *Hlo, const float *W3Thi, cons
     runs = (n_etiles + tiles_per_cta - 1) / tiles_per_cta;
     if (runs > 65535) { set_error("radial gemm: grid too large"); return E3_ERR_UNSUPPORTED; }
     static const int nprod = []() { const char *e = getenv("E3_RADIAL_PRODUCTS"); return (e && e[0] == '1') ? 1 : 3; }();
-    radial_gemm_fwd_kernel<<<dim3((unsigned)slabs, (unsigned)runs), 288, kGemmSmem, st>>>(Hhi, Hlo, W3Thi, W3Tlo, D, ldd, E, N, tiles_per_cta, nprod);
+    static const int dbg = []() { const char *e = getenv("E3_RADIAL_DBG"); return e ? atoi(e) : 0; }();
+    radial_gemm_fwd_kernel<<<dim3((unsigned)slabs, (unsigned)runs), 288, kGemmSmemFwd, st>>>(Hhi, Hlo, W3Thi, W3Tlo, D, ldd, E, N, tiles_per_cta, nprod, dbg);
     E3_CUDA_TRY(cudaGetLastError());
     return E3_OK;
 }
@@ -639,7 +648,7 @@ int launch_gemm_bwd(const float *A, long long lda, const float *Bhi, const float
 {
     static bool attr_set = false;
     if (!attr_set) {
-        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
+        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmemFwd));
         E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
         E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
         attr_set = true;
