@@ -345,7 +345,7 @@ def measure_config(k, args, world, rank, local, dev, steps, want_cpu, want_e2e):
         if rc != 0:
             raise RuntimeError(f"{what}: {L.e3_status_string(rc).decode()}: {L.e3_last_error().decode()}")
 
-    def step(timed_events=None):
+    def step(timed_events=None, sp=sp):
         def mark(name):
             if timed_events is not None:
                 e = torch.cuda.Event(enable_timing=True)
@@ -391,6 +391,29 @@ def measure_config(k, args, world, rank, local, dev, steps, want_cpu, want_e2e):
     barrier()
     clocks = sampler.stop()
     elapsed_ms, value = aggregate_replicas(t_start.elapsed_time(t_stop), E, steps, world, dev)
+
+    # the same step captured ONCE in a CUDA graph and replayed (the repeated-MD-step case: every launch is on the caller's stream and
+    # nothing synchronises, so the whole step is one graph); reported beside `value`, which stays the eager-launch number
+    graph_ms = None
+    try:
+        gstream = torch.cuda.Stream()
+        gstream.wait_stream(stream)
+        cgraph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(cgraph, stream=gstream):
+            step(sp=Ct.c_void_p(torch.cuda.current_stream().cuda_stream))
+        for _ in range(3):
+            cgraph.replay()
+        torch.cuda.synchronize()
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g0.record(stream)
+        for _ in range(steps):
+            cgraph.replay()
+        g1.record(stream)
+        torch.cuda.synchronize()
+        graph_ms = g0.elapsed_time(g1) / steps
+        del cgraph
+    except Exception as ex:                               # reported, never fatal: `value` does not depend on it
+        graph_ms = f"capture failed: {ex}"
 
     # per-call / per-kernel device times, measured live with events on the launching stream over
     # a second pass of the same steps (events between calls would otherwise perturb `value`)
@@ -455,7 +478,10 @@ def measure_config(k, args, world, rank, local, dev, steps, want_cpu, want_e2e):
                  "roofline": dom, "roofline_fwd": fwd_r, "tp_fwd_plus_vjp": tp,
                  "alu_peak": {"nominal_tflops": FP32_PEAK_TFLOPS, "measured_sustained_tflops": alu_meas,
                               "how": "148 SM x 128 lanes x 2 x 1.965 GHz; measured = e3_measure_fp32_peak (FFMA2 chains in registers, 0.3 s)"},
-                 "kernel_ms": kms, "kernel_info": {"fwd": plan.kernel_info(0), "bwd": plan.kernel_info(1)}}
+                 "kernel_ms": kms, "kernel_info": {"fwd": plan.kernel_info(0), "bwd": plan.kernel_info(1)},
+                 "graph_replay": ({"ms_per_step": graph_ms, "edges_per_s": E / (graph_ms * 1e-3),
+                                   "what": "the same step captured once in a CUDA graph and replayed `steps` times (this rank)"}
+                                  if isinstance(graph_ms, float) else {"error": graph_ms})}
 
     # NEXT-1: the same step with the weights GENERATED on the device by the radial network (PAPER.md L487-L491,
     # L539-L542) instead of being read as an input: radial fwd (hidden layers + tcgen05 3xTF32 GEMM) -> TP fwd -> TP VJP ->
@@ -640,7 +666,7 @@ def run_ours(args):
                 "ms_per_step": blk["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": blk["dtype"], "data": "synthetic"}
         for key in ("config", "clocks", "gpu_launches", "e2e", "roofline", "roofline_fwd", "tp_fwd_plus_vjp", "alu_peak", "kernel_ms",
-                    "kernel_info", "cpu_baseline", "radial", "next_rows"):
+                    "kernel_info", "cpu_baseline", "radial", "next_rows", "graph_replay"):
             line[key] = blk.get(key)
         line["csrc_sha"] = kernel_sources_sha()
         if sec is not None:
