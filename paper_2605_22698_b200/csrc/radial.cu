@@ -504,7 +504,7 @@ __device__ __forceinline__ void issue_chunk_t(uint32_t tmem_d, uint32_t sAhi, ui
 // with too few waves); rows x K chunk = 8192 elements per stage whatever the split
 template <int NT>
 __global__ void __launch_bounds__(256, 1) radial_gemm_bwd_kernel(const float *__restrict__ A, long long lda, const float *__restrict__ Bhi,
-                                                                 const float *__restrict__ Blo, long long ldb, float *__restrict__ D, long long M, long long Kt)
+                                                                 const float *__restrict__ Blo, long long ldb, float *__restrict__ D, long long M, long long Kt, int dbg)
 {
     constexpr int kBwdTiles = NT;
     constexpr int kBwdRows = 128 * kBwdTiles, kBwdK = 64 / kBwdTiles;
@@ -545,13 +545,13 @@ __global__ void __launch_bounds__(256, 1) radial_gemm_bwd_kernel(const float *__
         for (int j = 0; j < 8; ++j) {
             const int row = (j / kBwdPP) * 64 + r8, q = (j % kBwdPP) * 4 + q4;
             ra[j] = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (m0 + row < M && k0 + q * 4 + 4 <= Kt) ra[j] = __ldcs(reinterpret_cast<const float4 *>(A + (m0 + row) * lda + k0 + q * 4));
+            if (m0 + row < M && k0 + q * 4 + 4 <= Kt && !(dbg & 4)) ra[j] = __ldcs(reinterpret_cast<const float4 *>(A + (m0 + row) * lda + k0 + q * 4));
         }
 #pragma unroll
         for (int j = 0; j < kBwdPP; ++j) {
             const int q = j * 4 + q4;
             rbh[j] = make_float4(0.f, 0.f, 0.f, 0.f); rbl[j] = rbh[j];
-            if (k0 + q * 4 + 4 <= Kt) {
+            if (k0 + q * 4 + 4 <= Kt && !(dbg & 8)) {
                 rbh[j] = __ldg(reinterpret_cast<const float4 *>(Bhi + (long long)r8 * ldb + k0 + q * 4));
                 rbl[j] = __ldg(reinterpret_cast<const float4 *>(Blo + (long long)r8 * ldb + k0 + q * 4));
             }
@@ -577,16 +577,16 @@ __global__ void __launch_bounds__(256, 1) radial_gemm_bwd_kernel(const float *__
     };
     uint32_t ph0 = 0, ph1 = 0;
     auto step = [&](int kc, int buf, float4 (&ra)[8], float4 (&rbh)[kBwdPP], float4 (&rbl)[kBwdPP], uint32_t &ph) {
-        if (kc >= 2) {                                   // the MMAs of chunk kc - 2 must have finished reading this stage
+        if (kc >= 2 && !(dbg & 1)) {                     // the MMAs of chunk kc - 2 must have finished reading this stage
             mbar_wait_parity(mbar_s + buf * 8, ph);
             ph ^= 1u;
         }
-        store_chunk(buf, ra, rbh, rbl);
+        if (!(dbg & 2)) store_chunk(buf, ra, rbh, rbl);
         if (kc + 2 < k_chunks) load_chunk(kc + 2, ra, rbh, rbl);
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncthreads();
-        if (tid == 0) {
+        if (tid == 0 && !(dbg & 1)) {
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             const uint32_t b = smem_s + buf * kBwdStage;
 #pragma unroll
@@ -604,7 +604,7 @@ __global__ void __launch_bounds__(256, 1) radial_gemm_bwd_kernel(const float *__
     }
     {   // the last commit covers every MMA issued before it
         const int buf = (k_chunks - 1) & 1;
-        mbar_wait_parity(mbar_s + buf * 8, buf ? ph1 : ph0);
+        if (!(dbg & 1)) mbar_wait_parity(mbar_s + buf * 8, buf ? ph1 : ph0);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         float *stg = reinterpret_cast<float *>(smem + ((k_chunks & 1) ? kBwdStage : 0));       // the stage the last chunk did not use
         for (int t = 0; t < kBwdTiles; ++t)
@@ -658,8 +658,9 @@ int launch_gemm_bwd(const float *A, long long lda, const float *Bhi, const float
     const int nt = M >= 4LL * 148 * 512 ? 4 : 2;
     const long long grid = (M + 128 * nt - 1) / (128 * nt);
     if (grid > 0x7fffffffLL) { set_error("radial gemm: grid too large"); return E3_ERR_UNSUPPORTED; }
-    if (nt == 4) radial_gemm_bwd_kernel<4><<<(unsigned)grid, 256, kGemmSmem, st>>>(A, lda, Bhi, Blo, ldb, D, M, Kt);
-    else radial_gemm_bwd_kernel<2><<<(unsigned)grid, 256, kGemmSmem, st>>>(A, lda, Bhi, Blo, ldb, D, M, Kt);
+    static const int dbg = []() { const char *e = getenv("E3_RADIAL_DBG_BWD"); return e ? atoi(e) : 0; }();
+    if (nt == 4) radial_gemm_bwd_kernel<4><<<(unsigned)grid, 256, kGemmSmem, st>>>(A, lda, Bhi, Blo, ldb, D, M, Kt, dbg);
+    else radial_gemm_bwd_kernel<2><<<(unsigned)grid, 256, kGemmSmem, st>>>(A, lda, Bhi, Blo, ldb, D, M, Kt, dbg);
     E3_CUDA_TRY(cudaGetLastError());
     return E3_OK;
 }
