@@ -500,18 +500,20 @@ __device__ __forceinline__ void issue_chunk_t(uint32_t tmem_d, uint32_t sAhi, ui
     }
 }
 
-// kBwdTiles 128-row MMA tiles per CTA (template parameter NT: 4 for large edge counts, 2 when 512-row CTAs would leave the machine
-// with too few waves); rows x K chunk = 8192 elements per stage whatever the split
-template <int NT>
-__global__ void __launch_bounds__(256, 1) radial_gemm_bwd_kernel(const float *__restrict__ A, long long lda, const float *__restrict__ Bhi,
+// NT 128-row MMA tiles per CTA and K chunks of KC (template parameters; rows x KC = 8192 elements per stage for <4,16> and <2,32>, one
+// CTA per SM; <2,16,2> -- half the stage and register staging, TWO CTAs per SM -- was measured slower: 31.7 vs 27.4 ms on config 4)
+template <int NT, int KC, int MINB>
+__global__ void __launch_bounds__(256, MINB) radial_gemm_bwd_kernel(const float *__restrict__ A, long long lda, const float *__restrict__ Bhi,
                                                                  const float *__restrict__ Blo, long long ldb, float *__restrict__ D, long long M, long long Kt, int dbg)
 {
     constexpr int kBwdTiles = NT;
-    constexpr int kBwdRows = 128 * kBwdTiles, kBwdK = 64 / kBwdTiles;
+    constexpr int kBwdRows = 128 * kBwdTiles, kBwdK = KC;
+    constexpr int kBwdPA = NT * KC / 8;                                // 16-byte pieces of A per thread and chunk
+    constexpr int kBwdPlane = kBwdRows * kBwdK * 4;                    // one A plane (high or low parts)
     constexpr int kBwdQPR = kBwdK / 4, kBwdPP = kBwdQPR / 4;           // 16-byte quads per row; passes per 64-row block
     constexpr int kBwdSBO = kBwdQPR * 128;                             // bytes between groups of 8 rows
     constexpr int kBwdB = 64 * kBwdK * 4;                              // one B plane
-    constexpr int kBwdStage = 65536 + 2 * kBwdB;                       // stage: A hi 32 KB | A lo 32 KB | B hi | B lo
+    constexpr int kBwdStage = 2 * kBwdPlane + 2 * kBwdB;               // stage: A hi | A lo | B hi | B lo
     extern __shared__ __align__(1024) unsigned char smem[];
     __shared__ __align__(8) unsigned long long mbar[2];
     __shared__ uint32_t tmem_base_s;
@@ -538,11 +540,11 @@ __global__ void __launch_bounds__(256, 1) radial_gemm_bwd_kernel(const float *__
     // B [64 x 8 quads]: pass j: row = 8 warp + (lane & 7), quad = 4 j + (lane >> 3).  A warp covers 8 rows x 64 bytes: whole sectors in global
     // memory, 512 contiguous bytes in the canonical layout (conflict-free).
     const int r8 = warp * 8 + (lane & 7), q4 = lane >> 3;
-    float4 ra0[8], rbh0[kBwdPP], rbl0[kBwdPP], ra1[8], rbh1[kBwdPP], rbl1[kBwdPP];
-    auto load_chunk = [&](int kc, float4 (&ra)[8], float4 (&rbh)[kBwdPP], float4 (&rbl)[kBwdPP]) {
+    float4 ra0[kBwdPA], rbh0[kBwdPP], rbl0[kBwdPP], ra1[kBwdPA], rbh1[kBwdPP], rbl1[kBwdPP];
+    auto load_chunk = [&](int kc, float4 (&ra)[kBwdPA], float4 (&rbh)[kBwdPP], float4 (&rbl)[kBwdPP]) {
         const long long k0 = (long long)kc * kBwdK;
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
+        for (int j = 0; j < kBwdPA; ++j) {
             const int row = (j / kBwdPP) * 64 + r8, q = (j % kBwdPP) * 4 + q4;
             ra[j] = make_float4(0.f, 0.f, 0.f, 0.f);
             if (m0 + row < M && k0 + q * 4 + 4 <= Kt && !(dbg & 4)) ra[j] = __ldcs(reinterpret_cast<const float4 *>(A + (m0 + row) * lda + k0 + q * 4));
@@ -557,26 +559,26 @@ __global__ void __launch_bounds__(256, 1) radial_gemm_bwd_kernel(const float *__
             }
         }
     };
-    auto store_chunk = [&](int buf, const float4 (&ra)[8], const float4 (&rbh)[kBwdPP], const float4 (&rbl)[kBwdPP]) {
+    auto store_chunk = [&](int buf, const float4 (&ra)[kBwdPA], const float4 (&rbh)[kBwdPP], const float4 (&rbl)[kBwdPP]) {
         unsigned char *base = smem + buf * kBwdStage;
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
+        for (int j = 0; j < kBwdPA; ++j) {
             const int row = (j / kBwdPP) * 64 + r8, q = (j % kBwdPP) * 4 + q4;
             const float4 v = ra[j];
             const float4 h = make_float4(tf32_hi(v.x), tf32_hi(v.y), tf32_hi(v.z), tf32_hi(v.w));
             const uint32_t off = canon_off_sbo<kBwdSBO>(row, q * 4);
             *reinterpret_cast<float4 *>(base + off) = h;
-            *reinterpret_cast<float4 *>(base + 32768 + off) = make_float4(v.x - h.x, v.y - h.y, v.z - h.z, v.w - h.w);
+            *reinterpret_cast<float4 *>(base + kBwdPlane + off) = make_float4(v.x - h.x, v.y - h.y, v.z - h.z, v.w - h.w);
         }
 #pragma unroll
         for (int j = 0; j < kBwdPP; ++j) {
             const uint32_t off = canon_off_sbo<kBwdSBO>(r8, (j * 4 + q4) * 4);
-            *reinterpret_cast<float4 *>(base + 65536 + off) = rbh[j];
-            *reinterpret_cast<float4 *>(base + 65536 + kBwdB + off) = rbl[j];
+            *reinterpret_cast<float4 *>(base + 2 * kBwdPlane + off) = rbh[j];
+            *reinterpret_cast<float4 *>(base + 2 * kBwdPlane + kBwdB + off) = rbl[j];
         }
     };
     uint32_t ph0 = 0, ph1 = 0;
-    auto step = [&](int kc, int buf, float4 (&ra)[8], float4 (&rbh)[kBwdPP], float4 (&rbl)[kBwdPP], uint32_t &ph) {
+    auto step = [&](int kc, int buf, float4 (&ra)[kBwdPA], float4 (&rbh)[kBwdPP], float4 (&rbl)[kBwdPP], uint32_t &ph) {
         if (kc >= 2 && !(dbg & 1)) {                     // the MMAs of chunk kc - 2 must have finished reading this stage
             mbar_wait_parity(mbar_s + buf * 8, ph);
             ph ^= 1u;
@@ -592,7 +594,7 @@ __global__ void __launch_bounds__(256, 1) radial_gemm_bwd_kernel(const float *__
 #pragma unroll
             for (int t = 0; t < kBwdTiles; ++t)          // tile t: rows 128 t .. 128 t + 127 of the stage, accumulator columns 64 t ..
                 if (t == 0 || m0 + t * kTileM < M)
-                    issue_chunk_t<kBwdK / 8, kBwdSBO>(tmem + 64 * t, b + t * 16 * kBwdSBO, b + 32768 + t * 16 * kBwdSBO, b + 65536, b + 65536 + kBwdB, idesc, kc == 0);
+                    issue_chunk_t<kBwdK / 8, kBwdSBO>(tmem + 64 * t, b + t * 16 * kBwdSBO, b + kBwdPlane + t * 16 * kBwdSBO, b + 2 * kBwdPlane, b + 2 * kBwdPlane + kBwdB, idesc, kc == 0);
             asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(mbar_s + buf * 8) : "memory");
         }
     };
@@ -623,8 +625,8 @@ int launch_gemm_fwd(const float *Hhi, const float *Hlo, const float *W3Thi, cons
     static bool attr_set = false;
     if (!attr_set) {
         E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmemFwd));
-        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
-        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
+        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_kernel<4, 16, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
+        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_kernel<2, 32, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
         attr_set = true;
     }
     if (E <= 0) return E3_OK;
@@ -649,8 +651,8 @@ int launch_gemm_bwd(const float *A, long long lda, const float *Bhi, const float
     static bool attr_set = false;
     if (!attr_set) {
         E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmemFwd));
-        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
-        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
+        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_kernel<4, 16, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
+        E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_kernel<2, 32, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
         attr_set = true;
     }
     if (M <= 0) return E3_OK;
@@ -659,8 +661,8 @@ int launch_gemm_bwd(const float *A, long long lda, const float *Bhi, const float
     const long long grid = (M + 128 * nt - 1) / (128 * nt);
     if (grid > 0x7fffffffLL) { set_error("radial gemm: grid too large"); return E3_ERR_UNSUPPORTED; }
     static const int dbg = []() { const char *e = getenv("E3_RADIAL_DBG_BWD"); return e ? atoi(e) : 0; }();
-    if (nt == 4) radial_gemm_bwd_kernel<4><<<(unsigned)grid, 256, kGemmSmem, st>>>(A, lda, Bhi, Blo, ldb, D, M, Kt, dbg);
-    else radial_gemm_bwd_kernel<2><<<(unsigned)grid, 256, kGemmSmem, st>>>(A, lda, Bhi, Blo, ldb, D, M, Kt, dbg);
+    if (nt == 4) radial_gemm_bwd_kernel<4, 16, 1><<<(unsigned)grid, 256, kGemmSmem, st>>>(A, lda, Bhi, Blo, ldb, D, M, Kt, dbg);
+    else radial_gemm_bwd_kernel<2, 32, 1><<<(unsigned)grid, 256, kGemmSmem, st>>>(A, lda, Bhi, Blo, ldb, D, M, Kt, dbg);
     E3_CUDA_TRY(cudaGetLastError());
     return E3_OK;
 }
