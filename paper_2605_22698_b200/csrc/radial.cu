@@ -77,10 +77,12 @@ __device__ __forceinline__ void radial_feature(int k, float r, float rc, int p, 
     dfdr = db * u + b * du / rc;
 }
 
-// Hidden layers, forward and (BWD) their VJP.  A warp processes FOUR edges per pass; a lane owns hidden units `lane` and
-// `lane + 32` of all four.  The activations of the previous layer sit transposed in a per-warp shared-memory buffer [unit][edge], so
-// one broadcast 16-byte load serves eight FMAs (two units x four edges) beside the two weight loads: 3 LDS per 8 FMA instead of the
-// 2 LDS + 2 SHFL per 2 FMA of a one-edge-per-warp loop (which ran at 87 % of the LSU pipe, profiles/r02_radial.md).
+// Hidden layers, forward and (BWD) their VJP.  A warp processes EIGHT edges per pass; a lane owns hidden units `lane` and `lane + 32`
+// of all eight.  The activations of the previous layer sit transposed in a per-warp shared-memory buffer [unit][edge], so two broadcast
+// 16-byte loads serve sixteen FMAs (two units x eight edges) beside the two weight loads: 4 LDS per 16 FMA.  (One edge per warp: 2 LDS +
+// 2 SHFL per 2 FMA, 87 % of the LSU pipe; four edges per pass: 3 LDS per 8 FMA, still LSU-bound at 54 %, profiles/r02c_radial_cfg4_full.md.)
+constexpr int kEP = 8;          // edges per warp pass
+
 template <bool BWD>
 __global__ void __launch_bounds__(128) radial_hidden_kernel(const float *__restrict__ vec, long long E, int K, int p, float rc,
                                                             const float *__restrict__ W1, const float *__restrict__ W2, const float *__restrict__ W2T,
@@ -90,47 +92,69 @@ __global__ void __launch_bounds__(128) radial_hidden_kernel(const float *__restr
     float *W1s = hsm;                                   // [K][64]
     float *W2s = W1s + kMaxRbf * kH;                    // [64][64]
     float *W2Ts = W2s + kH * kH;                        // [64][64] transposed (BWD only)
-    float *W1Ts = W2Ts + (BWD ? kH * kH : 0);           // [64][16] transposed (BWD only)
-    float *wbuf = W1Ts + (BWD ? kH * kMaxRbf : 0);      // per warp: act[64][4] + feat[16][4] + dfeat[16][4]
+    float *W1Ts = W2Ts + (BWD ? kH * kH : 0);           // [64][4][4] (BWD only): W1[k = kk + 4 c][unit] at [unit][kk][c]
+    float *wbuf = W1Ts + (BWD ? kH * kMaxRbf : 0);      // per warp: act[64][8] + feat[16][8]
     for (int i = threadIdx.x; i < kMaxRbf * kH; i += blockDim.x) W1s[i] = i < K * kH ? W1[i] : 0.0f;
     for (int i = threadIdx.x; i < kH * kH; i += blockDim.x) { W2s[i] = W2[i]; if (BWD) W2Ts[i] = W2T[i]; }
-    if (BWD) for (int i = threadIdx.x; i < kH * kMaxRbf; i += blockDim.x) { const int u = i / kMaxRbf, k = i % kMaxRbf; W1Ts[i] = k < K ? W1[k * kH + u] : 0.0f; }
+    if (BWD)
+        for (int i = threadIdx.x; i < kH * kMaxRbf; i += blockDim.x) {
+            const int u = i / kMaxRbf, kq = (i % kMaxRbf) >> 2, c = i & 3, k = kq + 4 * c;
+            W1Ts[i] = k < K ? W1[k * kH + u] : 0.0f;
+        }
     __syncthreads();
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    float *act = wbuf + wib * (kH * 4 + 2 * kMaxRbf * 4), *feat = act + kH * 4, *dfeat = feat + kMaxRbf * 4;
+    float *act = wbuf + wib * (kH * kEP + kMaxRbf * kEP), *feat = act + kH * kEP;
     const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
-    const int el = lane >> 3, kk = lane & 7;            // this lane evaluates radial features kk and kk + 8 of edge el
-    for (long long e0 = warp * 4; e0 < E; e0 += nwarps * 4) {
+    const int el = lane >> 2, kk = lane & 3;            // this lane evaluates radial features kk, kk + 4, kk + 8, kk + 12 of edge el
+    for (long long e0 = warp * kEP; e0 < E; e0 += nwarps * kEP) {
         const long long em = e0 + el < E ? e0 + el : E - 1;
         const float vx = vec[3 * em], vy = vec[3 * em + 1], vz = vec[3 * em + 2];
         const float r = sqrtf(vx * vx + vy * vy + vz * vz);
-        float f0 = 0.0f, f1 = 0.0f, d0 = 0.0f, d1 = 0.0f;
-        if (kk < K) radial_feature(kk, r, rc, p, f0, d0);
-        if (kk + 8 < K) radial_feature(kk + 8, r, rc, p, f1, d1);
+        float f[4] = { 0.f, 0.f, 0.f, 0.f }, d[4] = { 0.f, 0.f, 0.f, 0.f };
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+            if (kk + 4 * c < K) radial_feature(kk + 4 * c, r, rc, p, f[c], d[c]);
         __syncwarp();
-        feat[kk * 4 + el] = f0; feat[(kk + 8) * 4 + el] = f1;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) feat[(kk + 4 * c) * kEP + el] = f[c];
         __syncwarp();
-        float a1[2][4] = {};
+        float a1[2][kEP] = {};
         for (int k = 0; k < K; ++k) {
-            const float4 fk = *reinterpret_cast<const float4 *>(feat + k * 4);
+            const float4 fa = *reinterpret_cast<const float4 *>(feat + k * kEP), fb = *reinterpret_cast<const float4 *>(feat + k * kEP + 4);
+            const float fk[kEP] = { fa.x, fa.y, fa.z, fa.w, fb.x, fb.y, fb.z, fb.w };
             const float w0 = W1s[k * kH + lane], w1 = W1s[k * kH + lane + 32];
-            a1[0][0] = fmaf(fk.x, w0, a1[0][0]); a1[0][1] = fmaf(fk.y, w0, a1[0][1]); a1[0][2] = fmaf(fk.z, w0, a1[0][2]); a1[0][3] = fmaf(fk.w, w0, a1[0][3]);
-            a1[1][0] = fmaf(fk.x, w1, a1[1][0]); a1[1][1] = fmaf(fk.y, w1, a1[1][1]); a1[1][2] = fmaf(fk.z, w1, a1[1][2]); a1[1][3] = fmaf(fk.w, w1, a1[1][3]);
+#pragma unroll
+            for (int q = 0; q < kEP; ++q) { a1[0][q] = fmaf(fk[q], w0, a1[0][q]); a1[1][q] = fmaf(fk[q], w1, a1[1][q]); }
         }
-        *reinterpret_cast<float4 *>(act + lane * 4) = make_float4(silu_f(a1[0][0]), silu_f(a1[0][1]), silu_f(a1[0][2]), silu_f(a1[0][3]));
-        *reinterpret_cast<float4 *>(act + (lane + 32) * 4) = make_float4(silu_f(a1[1][0]), silu_f(a1[1][1]), silu_f(a1[1][2]), silu_f(a1[1][3]));
+        auto put = [&](int unit, const float (&v)[kEP]) {
+            *reinterpret_cast<float4 *>(act + unit * kEP) = make_float4(v[0], v[1], v[2], v[3]);
+            *reinterpret_cast<float4 *>(act + unit * kEP + 4) = make_float4(v[4], v[5], v[6], v[7]);
+        };
+        {
+            float s0[kEP], s1[kEP];
+#pragma unroll
+            for (int q = 0; q < kEP; ++q) { s0[q] = silu_f(a1[0][q]); s1[q] = silu_f(a1[1][q]); }
+            put(lane, s0); put(lane + 32, s1);
+        }
         __syncwarp();
-        float a2[2][4] = {};
+        // out[u][q] = sum_i act[i][q] * Wm[i][u] for u = lane, lane + 32 (Wm = W2 forward, W2^T for the VJP)
+        auto layer = [&](const float *Wm, float (&o)[2][kEP]) {
+#pragma unroll
+            for (int q = 0; q < kEP; ++q) { o[0][q] = 0.f; o[1][q] = 0.f; }
 #pragma unroll 8
-        for (int i = 0; i < kH; ++i) {
-            const float4 h = *reinterpret_cast<const float4 *>(act + i * 4);
-            const float w0 = W2s[i * kH + lane], w1 = W2s[i * kH + lane + 32];
-            a2[0][0] = fmaf(h.x, w0, a2[0][0]); a2[0][1] = fmaf(h.y, w0, a2[0][1]); a2[0][2] = fmaf(h.z, w0, a2[0][2]); a2[0][3] = fmaf(h.w, w0, a2[0][3]);
-            a2[1][0] = fmaf(h.x, w1, a2[1][0]); a2[1][1] = fmaf(h.y, w1, a2[1][1]); a2[1][2] = fmaf(h.z, w1, a2[1][2]); a2[1][3] = fmaf(h.w, w1, a2[1][3]);
-        }
+            for (int i = 0; i < kH; ++i) {
+                const float4 ha = *reinterpret_cast<const float4 *>(act + i * kEP), hb = *reinterpret_cast<const float4 *>(act + i * kEP + 4);
+                const float h[kEP] = { ha.x, ha.y, ha.z, ha.w, hb.x, hb.y, hb.z, hb.w };
+                const float w0 = Wm[i * kH + lane], w1 = Wm[i * kH + lane + 32];
+#pragma unroll
+                for (int q = 0; q < kEP; ++q) { o[0][q] = fmaf(h[q], w0, o[0][q]); o[1][q] = fmaf(h[q], w1, o[1][q]); }
+            }
+        };
+        float a2[2][kEP];
+        layer(W2s, a2);
         if (!BWD) {
 #pragma unroll
-            for (int q = 0; q < 4; ++q)
+            for (int q = 0; q < kEP; ++q)
                 if (e0 + q < E) {      // h2 split into its TF32 high part and the exact remainder: the B operand of the output-layer GEMM
                     const float v0 = silu_f(a2[0][q]), v1 = silu_f(a2[1][q]);
                     const float h0 = __uint_as_float(__float_as_uint(v0) & 0xffffe000u), h1 = __uint_as_float(__float_as_uint(v1) & 0xffffe000u);
@@ -140,40 +164,38 @@ __global__ void __launch_bounds__(128) radial_hidden_kernel(const float *__restr
             continue;
         }
         // ---- VJP: dL/da2 -> dL/dh1 -> dL/da1 -> d f -> d r
-        float g2[2][4];
+        {
+            float g0[kEP], g1[kEP];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const long long eq = e0 + q < E ? e0 + q : E - 1;
-            g2[0][q] = dh2[eq * kH + lane] * dsilu_f(a2[0][q]);
-            g2[1][q] = dh2[eq * kH + lane + 32] * dsilu_f(a2[1][q]);
+            for (int q = 0; q < kEP; ++q) {
+                const long long eq = e0 + q < E ? e0 + q : E - 1;
+                g0[q] = dh2[eq * kH + lane] * dsilu_f(a2[0][q]);
+                g1[q] = dh2[eq * kH + lane + 32] * dsilu_f(a2[1][q]);
+            }
+            __syncwarp();
+            put(lane, g0); put(lane + 32, g1);
         }
         __syncwarp();
-        *reinterpret_cast<float4 *>(act + lane * 4) = make_float4(g2[0][0], g2[0][1], g2[0][2], g2[0][3]);
-        *reinterpret_cast<float4 *>(act + (lane + 32) * 4) = make_float4(g2[1][0], g2[1][1], g2[1][2], g2[1][3]);
+        float t[2][kEP];
+        layer(W2Ts, t);                                  // dL/dh1[i] = sum_j g2[j] W2[i][j]; W2T[j][i] is contiguous over the lanes
         __syncwarp();
-        float t[2][4] = {};
-#pragma unroll 8
-        for (int j = 0; j < kH; ++j) {                   // dL/dh1[i] = sum_j g2[j] W2[i][j]; W2T[j][i] is contiguous over the lanes
-            const float4 g = *reinterpret_cast<const float4 *>(act + j * 4);
-            const float w0 = W2Ts[j * kH + lane], w1 = W2Ts[j * kH + lane + 32];
-            t[0][0] = fmaf(g.x, w0, t[0][0]); t[0][1] = fmaf(g.y, w0, t[0][1]); t[0][2] = fmaf(g.z, w0, t[0][2]); t[0][3] = fmaf(g.w, w0, t[0][3]);
-            t[1][0] = fmaf(g.x, w1, t[1][0]); t[1][1] = fmaf(g.y, w1, t[1][1]); t[1][2] = fmaf(g.z, w1, t[1][2]); t[1][3] = fmaf(g.w, w1, t[1][3]);
+        {
+            float g0[kEP], g1[kEP];
+#pragma unroll
+            for (int q = 0; q < kEP; ++q) { g0[q] = t[0][q] * dsilu_f(a1[0][q]); g1[q] = t[1][q] * dsilu_f(a1[1][q]); }
+            put(lane, g0); put(lane + 32, g1);
         }
         __syncwarp();
-        *reinterpret_cast<float4 *>(act + lane * 4) = make_float4(t[0][0] * dsilu_f(a1[0][0]), t[0][1] * dsilu_f(a1[0][1]), t[0][2] * dsilu_f(a1[0][2]), t[0][3] * dsilu_f(a1[0][3]));
-        *reinterpret_cast<float4 *>(act + (lane + 32) * 4) = make_float4(t[1][0] * dsilu_f(a1[1][0]), t[1][1] * dsilu_f(a1[1][1]), t[1][2] * dsilu_f(a1[1][2]), t[1][3] * dsilu_f(a1[1][3]));
-        __syncwarp();
-        float df0 = 0.0f, df1 = 0.0f;                    // d f_k of edge el for k = kk, kk + 8: sum over the 64 units in ascending order
+        float df[4] = { 0.f, 0.f, 0.f, 0.f };            // d f_k of edge el for k = kk + 4 c: sum over the 64 units in ascending order
 #pragma unroll 8
         for (int i = 0; i < kH; ++i) {
-            const float g = act[i * 4 + el];
-            df0 = fmaf(g, W1Ts[i * kMaxRbf + kk], df0);
-            df1 = fmaf(g, W1Ts[i * kMaxRbf + kk + 8], df1);
+            const float g = act[i * kEP + el];
+            const float4 w = *reinterpret_cast<const float4 *>(W1Ts + i * kMaxRbf + kk * 4);
+            df[0] = fmaf(g, w.x, df[0]); df[1] = fmaf(g, w.y, df[1]); df[2] = fmaf(g, w.z, df[2]); df[3] = fmaf(g, w.w, df[3]);
         }
-        float dr = df0 * d0 + df1 * d1;
+        float dr = (df[0] * d[0] + df[1] * d[1]) + (df[2] * d[2] + df[3] * d[3]);
         dr += __shfl_xor_sync(0xffffffffu, dr, 1);
         dr += __shfl_xor_sync(0xffffffffu, dr, 2);
-        dr += __shfl_xor_sync(0xffffffffu, dr, 4);
         if (kk == 0 && e0 + el < E) {
             const long long e = e0 + el;
             const float inv = r > 0.0f ? 1.0f / r : 0.0f;
@@ -181,12 +203,11 @@ __global__ void __launch_bounds__(128) radial_hidden_kernel(const float *__restr
             if (accumulate) { gvec[3 * e] += gx; gvec[3 * e + 1] += gy; gvec[3 * e + 2] += gz; }
             else { gvec[3 * e] = gx; gvec[3 * e + 1] = gy; gvec[3 * e + 2] = gz; }
         }
-        (void)dfeat;
     }
 }
 
-constexpr int kHiddenSmemFwd = (kMaxRbf * kH + kH * kH + 4 * (kH * 4 + 2 * kMaxRbf * 4)) * 4;
-constexpr int kHiddenSmemBwd = (kMaxRbf * kH + 2 * kH * kH + kH * kMaxRbf + 4 * (kH * 4 + 2 * kMaxRbf * 4)) * 4;
+constexpr int kHiddenSmemFwd = (kMaxRbf * kH + kH * kH + 4 * (kH * kEP + kMaxRbf * kEP)) * 4;
+constexpr int kHiddenSmemBwd = (kMaxRbf * kH + 2 * kH * kH + kH * kMaxRbf + 4 * (kH * kEP + kMaxRbf * kEP)) * 4;
 
 // split W3 into TF32 high / low parts, both as [64][n_out] and transposed [n_out][64]
 __global__ void radial_split_w3_kernel(const float *__restrict__ W3, int n_out, float *__restrict__ hi, float *__restrict__ lo,
@@ -737,7 +758,7 @@ extern "C" int e3_radial_weights_fwd(const e3_radial *net, const float *vec, int
     if ((reinterpret_cast<uintptr_t>(weights) & 15u) || (reinterpret_cast<uintptr_t>(workspace) & 15u)) { set_error("e3_radial_weights_fwd: pointers must be 16-byte aligned"); return E3_ERR_INVALID_ARG; }
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     float *h2 = reinterpret_cast<float *>(workspace);
-    const long long blocks = std::min<long long>((n_edges + 15) / 16, 148LL * 8);
+    const long long blocks = std::min<long long>((n_edges + 31) / 32, 148LL * 8);
     radial_hidden_kernel<false><<<(unsigned)blocks, 128, kHiddenSmemFwd, st>>>(vec, n_edges, net->K, net->p, (float)net->rc, net->W1, net->W2, net->W2T, h2,
                                                                                 nullptr, nullptr, 0);
     E3_CUDA_TRY(cudaGetLastError());
@@ -756,7 +777,12 @@ extern "C" int e3_radial_weights_bwd(const e3_radial *net, const float *vec, int
     // dh2[E,64] = dw[E,n_out] * W3[64,n_out]^T : A = dw (K = n_out), B = W3 rows (K-major), one N tile, n_out / 64 K chunks
     int rc = launch_gemm_bwd(grad_weights, net->n_out, net->W3_hi, net->W3_lo, net->n_out, dh2, n_edges, net->n_out, st);
     if (rc != E3_OK) return rc;
-    const long long blocks = std::min<long long>((n_edges + 15) / 16, 148LL * 8);
+    const long long blocks = std::min<long long>((n_edges + 31) / 32, 148LL * 8);
+    static bool hidden_attr = false;
+    if (!hidden_attr) {          // 50 KB of dynamic shared memory: above the 48 KB default
+        E3_CUDA_TRY(cudaFuncSetAttribute(radial_hidden_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kHiddenSmemBwd));
+        hidden_attr = true;
+    }
     radial_hidden_kernel<true><<<(unsigned)blocks, 128, kHiddenSmemBwd, st>>>(vec, n_edges, net->K, net->p, (float)net->rc, net->W1, net->W2, net->W2T, nullptr,
                                                                                dh2, grad_vec, accumulate);
     E3_CUDA_TRY(cudaGetLastError());
