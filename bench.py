@@ -583,6 +583,47 @@ def measure_config(k, args, world, rank, local, dev, steps, want_cpu, want_e2e):
                                       "what": "one generated kernel pair per multiplicity class (64, 32) over the rows of the whole plan; weights = a prefix of the resident weight buffer"}}
         nq.destroy()
         del pos32, nb, xq, Gq, shq, outq, dxq, gshq, wsq, wq, dwq
+        # NEXT-3: MACE's symmetric contraction at correlation 2 on the graph's nodes: node features of the
+        # benchmark irreps, natural-parity paths up to out_lmax, 4 species.  One linear path per input irrep, one quadratic path per
+        # (i1 <= i2, L) allowed by the triangle rule.
+        sc_in = [(l, p_, C) for l, p_ in cfg.irreps_in]
+        sc_out, sc_paths = [], []
+        for i, (l, p_, m_) in enumerate(sc_in):
+            if l <= cfg.out_lmax:
+                sc_out.append((l, p_, m_)); sc_paths.append((i, -1, len(sc_out) - 1))
+        for i1, (l1, p1, m_) in enumerate(sc_in):
+            for i2 in range(i1, len(sc_in)):
+                l2, p2, _ = sc_in[i2]
+                for L3 in range(abs(l1 - l2), min(l1 + l2, cfg.out_lmax) + 1):
+                    if p1 * p2 == (-1) ** L3:
+                        sc_out.append((L3, p1 * p2, m_)); sc_paths.append((i1, i2, len(sc_out) - 1))
+        scn = B.SymCon(sc_in, sc_out, sc_paths, 4)
+        As = torch.randn((N, scn.in_dim * C), generator=gq, device=dev)
+        zs = torch.randint(0, 4, (N,), generator=gq, device=dev, dtype=torch.int32)
+        Ws = torch.randn((4, len(sc_paths), C), generator=gq, device=dev) / float(np.sqrt(len(sc_paths)))
+        Gs = torch.randn((N, scn.out_dim * C), generator=gq, device=dev)
+        sf = timed(lambda: scn.fwd(As, zs, Ws), nrep)
+        sb = timed(lambda: scn.bwd(As, zs, Ws, Gs), nrep)
+        sc_fB = N * (scn.in_dim + scn.out_dim) * C * 4
+        sc_bB = N * (2 * scn.in_dim + scn.out_dim) * C * 4
+        block["next_rows"]["symmetric_contraction"] = {
+            "paths": len(sc_paths), "cg_terms": scn.n_terms, "in_dim": scn.in_dim, "out_dim": scn.out_dim, "species": 4,
+            "ms_fwd": sf, "ms_bwd": sb, "nodes_per_s_fwd_plus_vjp": N / ((sf + sb) * 1e-3),
+            "algorithmic_bytes_fwd": sc_fB, "algorithmic_bytes_bwd": sc_bB,
+            "frac_of_hbm_fwd": sc_fB / (sf * 1e-3) / 1e9 / hbm_peak, "frac_of_hbm_bwd": sc_bB / (sb * 1e-3) / 1e9 / hbm_peak,
+            "what": "e3_symcon_fwd / _bwd (grad_feats + grad_weights) on the graph's nodes; per-node op, no gather: HBM-bound by the node rows"}
+        scn.destroy()
+        del As, zs, Ws, Gs
+        # NEXT-2: the second-order call with all three cotangents (a Hessian-row building block, section 5.2), when its extra
+        # weight-sized buffers fit (config 2)
+        if E * P * C * 4 < (2 << 30):
+            vx_, vY_, vw_ = torch.randn_like(x, dtype=torch.float32), torch.randn((E, plan.sh_dim), generator=gq, device=dev), torch.randn_like(w, dtype=torch.float32)
+            so = timed(lambda: B.e3_tp_scatter_vjp_vjp(plan, x, sh, w, snd, rcv, row_ptr, perm_s, col_ptr, N, G, vx_, vY_, vw_), max(3, nrep // 2))
+            block["next_rows"]["second_order"] = {"ms": so, "edges_per_s": E / (so * 1e-3),
+                                                  "first_order_fwd_plus_vjp_ms": kms["tp_scatter_fwd"] + kms["tp_scatter_bwd"],
+                                                  "what": "e3_tp_scatter_vjp_vjp with all three cotangents and all four outputs: 3 forward + 3 VJP launches of the plan's kernels "
+                                                          "and the adds (incl. the call's own buffer allocation in the binding)"}
+            del vx_, vY_, vw_
 
     # free the device-resident run before the host-buffer one (config 4 holds ~125 GB)
     del out, sh, gfe, gsh, gw, gvec, F, ws, gws, row_ptr, col_ptr, perm_s
