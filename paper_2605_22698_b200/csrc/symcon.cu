@@ -32,7 +32,16 @@ struct e3_symcon {
 
 namespace {
 
-constexpr int kChunks = 64;
+// node chunks of the grad_weights partial sums: about 32 nodes each (every thread walks its chunk's nodes serially), at least 64 chunks, at most
+// 4096 and at most 256 MB of partial sums.  A function of (N, table sizes) only: the summation order is fixed for a given problem.
+static int symcon_chunks(long long N, long long per_chunk_floats)
+{
+    long long c = (N + 31) / 32;
+    c = c < 64 ? 64 : (c > 4096 ? 4096 : c);
+    const long long cap = (256LL << 20) / 4 / (per_chunk_floats > 0 ? per_chunk_floats : 1);
+    if (c > cap) c = cap < 64 ? 64 : cap;
+    return (int)c;
+}
 
 __global__ void symcon_fwd_kernel(const float *__restrict__ A, const int32_t *__restrict__ species, const float *__restrict__ W, int C, int in_dim,
                                   int out_dim, int n_paths, int n_species, const int *__restrict__ ptr, const int *__restrict__ a1, const int *__restrict__ a2,
@@ -84,15 +93,15 @@ __global__ void symcon_bwd_feats_kernel(const float *__restrict__ A, const int32
     }
 }
 
-// grid (kChunks, ceil(n_paths * C / 128)): thread = (path, channel); partial[chunk][species][path][channel] over the chunk's nodes in ascending order
+// grid (chunks, ceil(n_paths * C / 128)): thread = (path, channel); partial[chunk][species][path][channel] over the chunk's nodes in ascending order
 __global__ void symcon_bwd_w_partial_kernel(const float *__restrict__ A, const int32_t *__restrict__ species, const float *__restrict__ G, int C, int in_dim,
-                                            int out_dim, int n_paths, int n_species, int N, const int *__restrict__ ptr, const int *__restrict__ a1,
+                                            int out_dim, int n_paths, int n_species, int N, int n_chunks, const int *__restrict__ ptr, const int *__restrict__ a1,
                                             const int *__restrict__ a2, const int *__restrict__ grow, const float *__restrict__ tc, float *__restrict__ partial)
 {
     const int idx = blockIdx.y * blockDim.x + threadIdx.x;
     if (idx >= n_paths * C) return;
     const int p = idx / C, u = idx % C;
-    const int per = (N + kChunks - 1) / kChunks, n0 = blockIdx.x * per, n1 = min(N, n0 + per);
+    const int per = (N + n_chunks - 1) / n_chunks, n0 = min(N, (int)blockIdx.x * per), n1 = min(N, n0 + per);
     float *dst = partial + (size_t)blockIdx.x * n_species * n_paths * C + idx;
     for (int s = 0; s < n_species; ++s) dst[(size_t)s * n_paths * C] = 0.0f;
     const int t0 = ptr[p], t1 = ptr[p + 1];
@@ -110,12 +119,12 @@ __global__ void symcon_bwd_w_partial_kernel(const float *__restrict__ A, const i
     }
 }
 
-__global__ void symcon_bwd_w_reduce_kernel(const float *__restrict__ partial, int total, float *__restrict__ dW)
+__global__ void symcon_bwd_w_reduce_kernel(const float *__restrict__ partial, int total, int n_chunks, float *__restrict__ dW)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= total) return;
     float acc = 0.0f;
-    for (int c = 0; c < kChunks; ++c) acc += partial[(size_t)c * total + i];
+    for (int c = 0; c < n_chunks; ++c) acc += partial[(size_t)c * total + i];
     dW[i] = acc;
 }
 
@@ -269,9 +278,9 @@ extern "C" int e3_symcon_fwd(const e3_symcon *sc, const float *feats, const int3
 
 extern "C" size_t e3_symcon_workspace_bytes(const e3_symcon *sc, int32_t n_nodes)
 {
-    (void)n_nodes;
     if (!sc) return 0;
-    return (size_t)kChunks * sc->n_species * sc->n_paths * sc->C * sizeof(float) + 256;
+    const long long per = (long long)sc->n_species * sc->n_paths * sc->C;
+    return (size_t)symcon_chunks(n_nodes, per) * per * sizeof(float) + 256;
 }
 
 extern "C" int e3_symcon_bwd(const e3_symcon *sc, const float *feats, const int32_t *species, const float *weights, int32_t n_nodes, const float *grad_out,
@@ -294,11 +303,11 @@ extern "C" int e3_symcon_bwd(const e3_symcon *sc, const float *feats, const int3
     if (grad_weights) {
         if (!workspace || workspace_bytes < e3_symcon_workspace_bytes(sc, n_nodes)) { set_error("e3_symcon_bwd: workspace too small"); return E3_ERR_WORKSPACE; }
         float *partial = reinterpret_cast<float *>(workspace);
-        const int pc = sc->n_paths * sc->C, total = sc->n_species * pc;
-        symcon_bwd_w_partial_kernel<<<dim3(kChunks, (unsigned)((pc + 127) / 128)), 128, 0, st>>>(
-            feats, species, grad_out, sc->C, sc->in_dim, sc->out_dim, sc->n_paths, sc->n_species, n_nodes, sc->w_ptr, sc->w_a1, sc->w_a2, sc->w_g, sc->w_c, partial);
+        const int pc = sc->n_paths * sc->C, total = sc->n_species * pc, chunks = symcon_chunks(n_nodes, total);
+        symcon_bwd_w_partial_kernel<<<dim3((unsigned)chunks, (unsigned)((pc + 127) / 128)), 128, 0, st>>>(
+            feats, species, grad_out, sc->C, sc->in_dim, sc->out_dim, sc->n_paths, sc->n_species, n_nodes, chunks, sc->w_ptr, sc->w_a1, sc->w_a2, sc->w_g, sc->w_c, partial);
         E3_CUDA_TRY(cudaGetLastError());
-        symcon_bwd_w_reduce_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(partial, total, grad_weights);
+        symcon_bwd_w_reduce_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(partial, total, chunks, grad_weights);
         E3_CUDA_TRY(cudaGetLastError());
     }
     return E3_OK;
