@@ -12,7 +12,11 @@ pytestmark = pytest.mark.gpu
 
 @pytest.mark.parametrize("C,lmax,out_lmax,N,S,natural", [(128, 3, 2, 1536, 4, True), (64, 2, 2, 700, 10, True), (33, 1, 1, 50, 1, False),
                                                           (8, 3, 3, 5, 3, False), (256, 2, 1, 64, 2, True)])
-def test_symmetric_contraction_against_oracle(C, lmax, out_lmax, N, S, natural):
+@pytest.mark.parametrize("jit", [True, False])
+def test_symmetric_contraction_against_oracle(C, lmax, out_lmax, N, S, natural, jit, monkeypatch):
+    """Both kernel families: the run-time specialised ones (default) and the table-driven fallback (E3_SYMCON_JIT=0)."""
+    if not jit:
+        monkeypatch.setenv("E3_SYMCON_JIT", "0")
     rng = np.random.default_rng(C + 10 * lmax + N)
     irreps_in = [(l, (-1) ** l, C) for l in range(lmax + 1)]
     irreps_out, paths = O.symcon_paths(irreps_in, out_lmax, natural_parity_only=natural)
