@@ -289,6 +289,10 @@ typedef struct { int i_in1; int i_in2; int i_out; } e3_pair_path;
 int e3_symcon_create(e3_symcon **sc, const e3_irrep *irreps_in, int n_in, const e3_irrep *irreps_out, int n_out,
                      const e3_pair_path *paths, int n_paths, int n_species);
 int e3_symcon_destroy(e3_symcon *sc);
+/* Build-time check (host only, no device needed): generates and compiles the specialised kernels of this path table for sm_100a; returns the
+ * forward kernel's registers and spill bytes.  Same validation and status codes as e3_symcon_create. */
+int e3_symcon_jit_check(const e3_irrep *irreps_in, int n_in, const e3_irrep *irreps_out, int n_out, const e3_pair_path *paths, int n_paths,
+                        int *fwd_regs, int *fwd_spill);
 int e3_symcon_dims(const e3_symcon *sc, int *in_dim, int *out_dim, int *n_paths, int *n_terms);
 int e3_symcon_fwd(const e3_symcon *sc, const float *feats, const int32_t *species, const float *weights, int32_t n_nodes,
                   float *out, e3_stream stream);

@@ -25,7 +25,7 @@ SYMBOLS = [
     "e3_graph_prepare", "e3_sh_fwd", "e3_sh_bwd", "e3_tp_scatter_fwd", "e3_bwd_workspace_bytes", "e3_tp_scatter_bwd",
     "e3_force_reduce", "e3_profile_set_mid_event", "e3_measure_fp32_peak", "e3_session_create", "e3_session_destroy", "e3_session_run_host",
     "e3_vjp_vjp_workspace_bytes", "e3_tp_scatter_vjp_vjp", "e3_sh_bwd_bwd",
-    "e3_symcon_create", "e3_symcon_destroy", "e3_symcon_dims", "e3_symcon_fwd", "e3_symcon_workspace_bytes", "e3_symcon_bwd",
+    "e3_symcon_create", "e3_symcon_jit_check", "e3_symcon_destroy", "e3_symcon_dims", "e3_symcon_fwd", "e3_symcon_workspace_bytes", "e3_symcon_bwd",
     "e3_neighbor_workspace_bytes", "e3_neighbor_build", "e3_shard_ranges", "e3_shard_localize",
     "e3_radial_create", "e3_radial_destroy", "e3_radial_workspace_bytes", "e3_radial_weights_fwd", "e3_radial_weights_bwd",
 ]
@@ -475,3 +475,12 @@ def e3_shard_localize(senders_h, receivers_h, n_nodes, lo, hi):
     _check(lib().e3_shard_localize(*args, C.byref(e_lo), C.byref(e_hi), _hptr(halo, np.int32), C.byref(nh), _hptr(sl, np.int32),
                                    _hptr(rl, np.int32)), "e3_shard_localize")
     return dict(lo=lo, hi=hi, e_lo=e_lo.value, e_hi=e_hi.value, halo=halo[:nh.value].copy(), senders_local=sl[:n], receivers_local=rl[:n])
+
+
+def e3_symcon_jit_check(irreps_in, irreps_out, paths):
+    """Build-time compile check of the specialised symmetric-contraction kernels (no device needed)."""
+    pp = (_PairPath * len(paths))(*[_PairPath(*map(int, t)) for t in paths])
+    regs, spill = C.c_int(), C.c_int()
+    _check(lib().e3_symcon_jit_check(_irreps(irreps_in), len(irreps_in), _irreps(irreps_out), len(irreps_out), pp, len(paths),
+                                     C.byref(regs), C.byref(spill)), "e3_symcon_jit_check")
+    return dict(fwd_regs=regs.value, fwd_spill=spill.value)

@@ -310,13 +310,14 @@ extern "C" int e3_symcon_destroy(e3_symcon *sc)
     return E3_OK;
 }
 
-extern "C" int e3_symcon_create(e3_symcon **out, const e3_irrep *irreps_in, int n_in, const e3_irrep *irreps_out, int n_out, const e3_pair_path *paths,
-                                int n_paths, int n_species)
+// device = false: build-time check only (host CG instantiation, generation + NVRTC compilation, nothing uploaded or loaded)
+static int symcon_create_impl(e3_symcon **out, const e3_irrep *irreps_in, int n_in, const e3_irrep *irreps_out, int n_out, const e3_pair_path *paths,
+                              int n_paths, int n_species, bool device, int *regs, int *spill)
 {
     if (!out || !irreps_in || !irreps_out || !paths || n_in < 1 || n_out < 1 || n_paths < 1 || n_species < 1) { set_error("e3_symcon_create: bad arguments"); return E3_ERR_INVALID_ARG; }
     *out = nullptr;
     int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); set_error("e3_symcon_create: no CUDA device (no CPU fallback)"); return E3_ERR_CUDA; }
+    if (device && (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1)) { cudaGetLastError(); set_error("e3_symcon_create: no CUDA device (no CPU fallback)"); return E3_ERR_CUDA; }
     const int C = irreps_in[0].mul;
     std::vector<int> in_off(n_in), out_off(n_out);
     int in_dim = 0, out_dim = 0;
@@ -347,9 +348,18 @@ extern "C" int e3_symcon_create(e3_symcon **out, const e3_irrep *irreps_in, int 
         }
     }
     std::vector<std::vector<double>> dense;
-    if (!triples.empty()) {
+    if (!triples.empty() && device) {
         int rc = launch_cg_planner(triples.data(), (int)triples.size() / 3, dense);
         if (rc != E3_OK) return rc;
+    } else {
+        for (size_t q = 0; q + 2 < triples.size(); q += 3) {
+            const int l1 = triples[q], l2 = triples[q + 1], L = triples[q + 2];
+            std::vector<double> d;
+            for (int a = 0; a <= 2 * l1; ++a)
+                for (int b = 0; b <= 2 * l2; ++b)
+                    for (int c = 0; c <= 2 * L; ++c) d.push_back(cg_real_host(l1, l2, L, a, b, c));
+            dense.push_back(d);
+        }
     }
     struct Term { int a1, a2, grow, p; float c; };
     std::vector<Term> terms;
@@ -394,21 +404,22 @@ extern "C" int e3_symcon_create(e3_symcon **out, const e3_irrep *irreps_in, int 
         for (const Term &t : terms) if (t.p == p) { wa1.push_back(t.a1); wa2.push_back(t.a2); wg.push_back(t.grow); wc.push_back(t.c); }
         wptr[p + 1] = (int)wa1.size();
     }
-    int rc = upload(&sc->f_ptr, fptr);
-    if (rc == E3_OK) rc = upload(&sc->f_a1, fa1);
-    if (rc == E3_OK) rc = upload(&sc->f_a2, fa2);
-    if (rc == E3_OK) rc = upload(&sc->f_p, fp);
-    if (rc == E3_OK) rc = upload(&sc->f_c, fc);
-    if (rc == E3_OK) rc = upload(&sc->b_ptr, bptr);
-    if (rc == E3_OK) rc = upload(&sc->b_other, bo);
-    if (rc == E3_OK) rc = upload(&sc->b_g, bg);
-    if (rc == E3_OK) rc = upload(&sc->b_p, bp);
-    if (rc == E3_OK) rc = upload(&sc->b_c, bc);
-    if (rc == E3_OK) rc = upload(&sc->w_ptr, wptr);
-    if (rc == E3_OK) rc = upload(&sc->w_a1, wa1);
-    if (rc == E3_OK) rc = upload(&sc->w_a2, wa2);
-    if (rc == E3_OK) rc = upload(&sc->w_g, wg);
-    if (rc == E3_OK) rc = upload(&sc->w_c, wc);
+    int rc = E3_OK;
+    if (device) rc = upload(&sc->f_ptr, fptr);
+    if (device && rc == E3_OK) rc = upload(&sc->f_a1, fa1);
+    if (device && rc == E3_OK) rc = upload(&sc->f_a2, fa2);
+    if (device && rc == E3_OK) rc = upload(&sc->f_p, fp);
+    if (device && rc == E3_OK) rc = upload(&sc->f_c, fc);
+    if (device && rc == E3_OK) rc = upload(&sc->b_ptr, bptr);
+    if (device && rc == E3_OK) rc = upload(&sc->b_other, bo);
+    if (device && rc == E3_OK) rc = upload(&sc->b_g, bg);
+    if (device && rc == E3_OK) rc = upload(&sc->b_p, bp);
+    if (device && rc == E3_OK) rc = upload(&sc->b_c, bc);
+    if (device && rc == E3_OK) rc = upload(&sc->w_ptr, wptr);
+    if (device && rc == E3_OK) rc = upload(&sc->w_a1, wa1);
+    if (device && rc == E3_OK) rc = upload(&sc->w_a2, wa2);
+    if (device && rc == E3_OK) rc = upload(&sc->w_g, wg);
+    if (device && rc == E3_OK) rc = upload(&sc->w_c, wc);
     // specialised kernels: one NVRTC compilation holds all three (E3_SYMCON_JIT=0 keeps the table-driven ones)
     const char *je = getenv("E3_SYMCON_JIT");
     if (rc == E3_OK && !(je && je[0] == '0') && terms.size() <= 6000) {
@@ -421,15 +432,30 @@ extern "C" int e3_symcon_create(e3_symcon **out, const e3_irrep *irreps_in, int 
         if (rc == E3_OK) {
             sc->jbf = sc->jfwd; sc->jbf.name = "e3_sc_bwd_feats"; sc->jbf.lib = nullptr; sc->jbf.fn = nullptr;
             sc->jbw = sc->jfwd; sc->jbw.name = "e3_sc_bwd_w"; sc->jbw.lib = nullptr; sc->jbw.fn = nullptr;
-            rc = jit_load(sc->jfwd);
-            if (rc == E3_OK) rc = jit_load(sc->jbf);
-            if (rc == E3_OK) rc = jit_load(sc->jbw);
-            sc->jit = rc == E3_OK;
+            if (regs) *regs = sc->jfwd.regs;
+            if (spill) *spill = sc->jfwd.spill;
+            if (device) rc = jit_load(sc->jfwd);
+            if (device && rc == E3_OK) rc = jit_load(sc->jbf);
+            if (device && rc == E3_OK) rc = jit_load(sc->jbw);
+            sc->jit = device && rc == E3_OK;
         }
     }
-    if (rc != E3_OK) { e3_symcon_destroy(sc); return rc; }
+    if (rc != E3_OK || !device) { e3_symcon_destroy(sc); return rc; }
     *out = sc;
     return E3_OK;
+}
+
+extern "C" int e3_symcon_create(e3_symcon **out, const e3_irrep *irreps_in, int n_in, const e3_irrep *irreps_out, int n_out, const e3_pair_path *paths,
+                                int n_paths, int n_species)
+{
+    return symcon_create_impl(out, irreps_in, n_in, irreps_out, n_out, paths, n_paths, n_species, true, nullptr, nullptr);
+}
+
+extern "C" int e3_symcon_jit_check(const e3_irrep *irreps_in, int n_in, const e3_irrep *irreps_out, int n_out, const e3_pair_path *paths, int n_paths,
+                                   int *fwd_regs, int *fwd_spill)
+{
+    e3_symcon *tmp = nullptr;
+    return symcon_create_impl(&tmp, irreps_in, n_in, irreps_out, n_out, paths, n_paths, 1, false, fwd_regs, fwd_spill);
 }
 
 extern "C" int e3_symcon_dims(const e3_symcon *sc, int *in_dim, int *out_dim, int *n_paths, int *n_terms)

@@ -95,3 +95,16 @@ def test_product_package_never_imports_the_oracle():
             if f.endswith((".py", ".cu", ".cpp", ".h")):
                 src = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in src and "from oracle" not in src and "e3_oracle" not in src, f
+
+
+def test_symcon_jit_check_compiles_and_validates():
+    """NEXT-3: the specialised symmetric-contraction kernels are generated and compiled for sm_100a without a device."""
+    C = 8
+    ii = [(0, 1, C), (1, -1, C), (2, 1, C)]
+    io = [(0, 1, C), (1, -1, C), (2, 1, C), (0, 1, C), (2, 1, C), (1, -1, C)]
+    pp = [(0, -1, 0), (1, -1, 1), (2, -1, 2), (1, 1, 3), (1, 1, 4), (1, 2, 5)]
+    r = B.e3_symcon_jit_check(ii, io, pp)
+    assert r["fwd_regs"] > 0 and r["fwd_spill"] == 0, r
+    with pytest.raises(B.E3Error) as e:
+        B.e3_symcon_jit_check([(0, 1, C)], [(3, -1, C)], [(0, 0, 0)])        # 0 x 0 -> 3: triangle rule
+    assert e.value.status == B.E3_ERR_BAD_PATH
