@@ -150,3 +150,73 @@ def test_nequip_multiplicities_on_the_config2_graph():
     _, errs = _run_both(pl, (in_size, sh_dim, out_size, w_size), g.senders, g.receivers, g.vec, x, w, G)
     print({k: f"{v:.2e}" for k, v in errs.items()})
     assert errs["out"] <= TOL_FWD and max(errs["dx"], errs["dY"], errs["dw"]) <= TOL_VJP, errs
+
+
+def _random_mul_case(rng):
+    """Random plan with per-irrep multiplicities (multiples of 4): random irreps of both parities, a random subset of the allowed paths
+    (some input irreps end up unread), sometimes several paths of one multiplicity adding into one output block (A6), ragged graph."""
+    muls = [int(m) for m in rng.choice([4, 8, 12, 16, 32, 64, 128], size=int(rng.integers(2, 4)), replace=False)]
+    irreps_in = []
+    for l in range(int(rng.integers(1, 4)) + 1):
+        for par in (1, -1):
+            if rng.random() < 0.6:
+                irreps_in.append((l, par, int(rng.choice(muls))))
+    if len(set(t[2] for t in irreps_in)) < 2:
+        irreps_in = [(0, 1, muls[0]), (1, -1, muls[1])]
+    sh_lmax, out_lmax = int(rng.integers(1, 4)), int(rng.integers(0, 4))
+    irreps_out, paths = O.all_paths(irreps_in, sh_lmax, out_lmax, bool(rng.random() < 0.3))
+    keep = [i for i in range(len(paths)) if rng.random() < 0.75]
+    if len(keep) < 2:
+        return None
+    paths = [paths[i] for i in keep]
+    used = sorted(set(p[2] for p in paths))
+    remap = {o: k for k, o in enumerate(used)}
+    irreps_out = [irreps_out[o] for o in used]
+    paths = [(a, b, remap[c]) for a, b, c in paths]
+    if rng.random() < 0.4:                                                   # shared output blocks: same (l, parity, mul) only
+        first, new_out, m = {}, [], {}
+        for k, io in enumerate(irreps_out):
+            if io in first and rng.random() < 0.7:
+                m[k] = first[io]
+            else:
+                first.setdefault(io, len(new_out))
+                m[k] = len(new_out)
+                new_out.append(io)
+        irreps_out, paths = new_out, [(a, b, m[c]) for a, b, c in paths]
+    if len(set(irreps_in[p[0]][2] for p in paths)) < 1:
+        return None
+    in_size, sh_dim, out_size, w_size = O.tp_mul_dims(irreps_in, sh_lmax, irreps_out, paths)
+    n = int(rng.integers(1, 60))
+    snd, rcv = _ragged_graph(rng, n, int(rng.integers(1, 30)))
+    e = len(snd)
+    vec = (rng.normal(size=(e, 3)) * 2).astype(np.float32)
+    x = rng.normal(size=(n, in_size)).astype(np.float32)
+    w = (rng.normal(size=(e, w_size)) / np.sqrt(len(paths))).astype(np.float32)
+    G = rng.normal(size=(n, out_size)).astype(np.float32)
+    return (irreps_in, sh_lmax, irreps_out, paths), (in_size, sh_dim, out_size, w_size), snd, rcv, vec, x, w, G
+
+
+@pytest.mark.parametrize("block", range(3))
+def test_random_plans_with_unequal_multiplicities(block, monkeypatch):
+    tunes = ["", "fwd_split=2,bwd_split=2", "bwd_role_cost=1", "v2=0", "rows=12", "bwd_overlap=3"]
+    done = 0
+    for it in range(16):
+        rng = np.random.default_rng(991000 + 100 * block + it)
+        case = _random_mul_case(rng)
+        if case is None:
+            continue
+        pl, sizes, *data = case
+        tune = tunes[int(rng.integers(0, len(tunes)))]
+        if tune:
+            monkeypatch.setenv("E3_TUNE", tune)
+        else:
+            monkeypatch.delenv("E3_TUNE", raising=False)
+        storage = "bf16" if rng.random() < 0.25 else "f32"
+        try:
+            _, errs = _run_both(pl, sizes, *data, storage=storage)
+        except Exception as ex:
+            raise AssertionError(f"block {block} it {it}: in={pl[0]} sh={pl[1]} out={pl[2]} paths={pl[3]} tune={tune!r} {storage}: {ex}") from ex
+        bar_f, bar_v = (TOL_BF16, TOL_BF16) if storage == "bf16" else (TOL_FWD, TOL_VJP)
+        assert errs["out"] <= bar_f and max(errs["dx"], errs["dY"], errs["dw"]) <= bar_v, (block, it, pl, tune, storage, errs)
+        done += 1
+    assert done >= 10
