@@ -474,7 +474,7 @@ void plan_make_roles(e3_plan &pl)
     tune_get("fwd_v3_bulk", pl.fwd_v3_bulk);
     pl.fwd_v3 = 0;             // opt-in (E3_TUNE fwd_v3=1): measured no faster than the second generation (experiment viii)
     tune_get("fwd_v3", pl.fwd_v3);
-    if (!pl.v2 || !v3_eligible(pl)) pl.fwd_v3 = 0;
+    if (!pl.v2 || !v3_eligible(pl) || !pl.in_base.empty()) pl.fwd_v3 = 0;      // the v3 generator knows the regular layout only (not the sub-plans of a composite)
     tune_get("team", pl.fwd_tw); tune_get("fwd_v3_depth", pl.fwd_v3_depth); tune_get("fwd_v3_lag", pl.fwd_v3_lag); tune_get("fwd_v3_chunk", pl.fwd_v3_chunk); tune_get("fwd_v3_bulk", pl.fwd_v3_bulk);
     pl.fwd_tw = std::max(1, std::min(4, pl.fwd_tw));
     pl.fwd_v3_lag = std::max(1, std::min(2, pl.fwd_v3_lag));

@@ -198,7 +198,7 @@ def _random_mul_case(rng):
 
 @pytest.mark.parametrize("block", range(3))
 def test_random_plans_with_unequal_multiplicities(block, monkeypatch):
-    tunes = ["", "fwd_split=2,bwd_split=2", "bwd_role_cost=1", "v2=0", "rows=12", "bwd_overlap=3"]
+    tunes = ["", "fwd_split=2,bwd_split=2", "bwd_role_cost=1", "v2=0", "rows=12", "bwd_overlap=3", "fwd_v3=1"]
     done = 0
     for it in range(16):
         rng = np.random.default_rng(991000 + 100 * block + it)
