@@ -336,6 +336,23 @@ int e3_shard_ranges(const int32_t *receivers_h, int64_t n_edges, int32_t n_nodes
 int e3_shard_localize(const int32_t *senders_h, const int32_t *receivers_h, int64_t n_edges, int32_t n_nodes, int32_t lo, int32_t hi,
                       int64_t *e_lo, int64_t *e_hi, int32_t *halo, int32_t *n_halo, int32_t *senders_local, int32_t *receivers_local);
 
+/* ---------------------------------------------------------------------------------------------
+ * Graph preparation without any allocation (same operation, arguments and results as e3_graph_prepare: SURVEY 8(a) a3, readings
+ * A11/A14/A15), for callers that cannot call cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it.  The scratch of e3_graph_prepare lives in a static device array of e3_graph_noalloc_capacity_bytes() = 32 MiB that every
+ * GPU loading the library holds until the process exits; the call allocates and frees nothing (no cudaMalloc / cudaFree, no
+ * allocating library routine).  Limit: e3_graph_workspace_bytes(n_edges, n_nodes) <= the capacity, i.e. n_edges + n_nodes <=
+ * 8 388 600; beyond it E3_ERR_WORKSPACE is returned with the sizes in e3_last_error() and nothing is launched.
+ * All pointers are device pointers owned by the caller (row_ptr[N+1], perm_s[E], col_ptr[N+1]); the device of `stream` must be
+ * current.  validate != 0 synchronises `stream` as in e3_graph_prepare.
+ * SHARING: every call on a device uses the same array.  Calls that overlap on the GPU (different streams, or threads that do not
+ * order their calls) race on it and give undefined results; calls on one stream are ordered and safe.  The array keeps the last
+ * call's contents; the call clears or overwrites everything it reads, so that is harmless.
+ * -------------------------------------------------------------------------------------------*/
+size_t e3_graph_noalloc_capacity_bytes(void);
+int e3_graph_prepare_noalloc(const int32_t *senders, const int32_t *receivers, int64_t n_edges, int32_t n_nodes,
+                             int32_t *row_ptr, int32_t *perm_s, int32_t *col_ptr, int validate, e3_stream stream);
+
 #ifdef __cplusplus
 }
 #endif

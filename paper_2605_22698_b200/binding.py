@@ -28,6 +28,7 @@ SYMBOLS = [
     "e3_symcon_create", "e3_symcon_jit_check", "e3_symcon_destroy", "e3_symcon_dims", "e3_symcon_fwd", "e3_symcon_workspace_bytes", "e3_symcon_bwd",
     "e3_neighbor_workspace_bytes", "e3_neighbor_build", "e3_shard_ranges", "e3_shard_localize",
     "e3_radial_create", "e3_radial_destroy", "e3_radial_workspace_bytes", "e3_radial_weights_fwd", "e3_radial_weights_bwd",
+    "e3_graph_noalloc_capacity_bytes", "e3_graph_prepare_noalloc",
 ]
 
 
@@ -59,6 +60,8 @@ def lib():
         L.e3_last_error.restype = C.c_char_p
         L.e3_graph_workspace_bytes.restype = C.c_size_t
         L.e3_graph_workspace_bytes.argtypes = [C.c_int64, C.c_int32]
+        L.e3_graph_noalloc_capacity_bytes.restype = C.c_size_t
+        L.e3_graph_noalloc_capacity_bytes.argtypes = []
         L.e3_bwd_workspace_bytes.restype = C.c_size_t
         L.e3_bwd_workspace_bytes.argtypes = [C.c_void_p, C.c_int64, C.c_int32]
         L.e3_vjp_vjp_workspace_bytes.restype = C.c_size_t
@@ -198,6 +201,21 @@ def e3_graph_prepare(senders, receivers, n_nodes, validate=False, stream=None):
                                   _ptr(perm_s), _ptr(col_ptr), _ptr(ws), C.c_size_t(nbytes), int(bool(validate)),
                                   _stream(stream)), "e3_graph_prepare")
     return row_ptr, perm_s, col_ptr
+
+
+def e3_graph_noalloc_capacity_bytes():
+    return int(lib().e3_graph_noalloc_capacity_bytes())
+
+
+def e3_graph_prepare_noalloc(senders, receivers, n_nodes, row_ptr, perm_s, col_ptr, validate=False, stream=None):
+    """e3_graph_prepare into caller-owned outputs with the library's static scratch: nothing is allocated, here or in the library."""
+    _dev(senders, torch.int32); _dev(receivers, torch.int32)
+    _dev(row_ptr, torch.int32); _dev(perm_s, torch.int32); _dev(col_ptr, torch.int32)
+    E = senders.numel()
+    if row_ptr.numel() < n_nodes + 1 or col_ptr.numel() < n_nodes + 1 or perm_s.numel() < E or receivers.numel() != E:
+        raise ValueError("e3_graph_prepare_noalloc: output tensors too small")
+    _check(lib().e3_graph_prepare_noalloc(_ptr(senders), _ptr(receivers), C.c_int64(E), C.c_int32(n_nodes), _ptr(row_ptr),
+                                          _ptr(perm_s), _ptr(col_ptr), int(bool(validate)), _stream(stream)), "e3_graph_prepare_noalloc")
 
 
 def e3_sh_fwd(plan: Plan, vec, out=None, stream=None):

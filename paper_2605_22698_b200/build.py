@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libe3b200.so")
-SOURCES = ["plan.cu", "kernels.cu", "api.cu", "radial.cu", "symcon.cu", "neighbor.cu", "codegen.cpp", "codegen2.cpp", "jit.cpp", "shard.cpp"]
+SOURCES = ["plan.cu", "kernels.cu", "api.cu", "radial.cu", "symcon.cu", "neighbor.cu", "noalloc.cu", "codegen.cpp", "codegen2.cpp", "jit.cpp", "shard.cpp"]
 CUDA_HOME = os.environ.get("CUDA_HOME", "/usr/local/cuda")
 
 
