@@ -39,19 +39,35 @@ struct e3_symcon {
     // run-time specialised kernels (the CG terms as straight-line code with immediate coefficients, rows in registers); the table-driven
     // kernels above stay as the fallback for very long term lists and for E3_SYMCON_JIT=0
     bool jit = false;
-    e3::JitKernel jfwd, jbf, jbw;
+    e3::JitKernel jfwd, jbf, jbw, jbb;
+    int acc_smem = 0;      // bytes of the node-chunk kernels' shared accumulators (n_species * n_paths * 128 floats); 0 = too large, table-driven grad_weights
+    int slots = 0;         // CTAs of e3_sc_bwd_both resident on the device at once (the chunk count is rounded to whole waves of them)
 };
 
 namespace {
 
-// node chunks of the grad_weights partial sums: about 32 nodes each (every thread walks its chunk's nodes serially), at least 64 chunks, at most
-// 4096 and at most 256 MB of partial sums.  A function of (N, table sizes) only: the summation order is fixed for a given problem.
-static int symcon_chunks(long long N, long long per_chunk_floats)
+// node chunks of the grad_weights partial sums: a thread (chunk, channel) walks its chunk's nodes serially.  About 32 nodes per chunk; for
+// small N fewer (down to 4) so that the launch still covers the machine; the number of 128-thread CTAs is rounded up to whole waves of
+// `slots` resident CTAs (equal-length CTAs: a partial last wave costs a whole one); at most 256 MB of partial sums.  A function of
+// (N, C, table sizes, device) only: the summation order is fixed for a given problem on a given device type.
+static int symcon_chunks(long long N, long long C, long long per_chunk_floats, long long slots)
 {
+    if (N <= 0) return 1;
+    if (C < 1) C = 1;
+    if (slots < 1) slots = 592;
     long long c = (N + 31) / 32;
-    c = c < 64 ? 64 : (c > 4096 ? 4096 : c);
+    long long ctas = (c * C + 127) / 128;
+    if (ctas < slots) {                                   // small problem: shorter chunks, one wave at most
+        const long long c4 = (N + 3) / 4, ctas4 = (c4 * C + 127) / 128;
+        ctas = ctas4 < slots ? ctas4 : slots;
+    } else {
+        ctas = ((ctas + slots - 1) / slots) * slots;
+    }
+    c = (ctas * 128) / C;
+    if (c < 1) c = 1;
+    if (c > N) c = N;
     const long long cap = (256LL << 20) / 4 / (per_chunk_floats > 0 ? per_chunk_floats : 1);
-    if (c > cap) c = cap < 64 ? 64 : cap;
+    if (c > cap) c = cap < 1 ? 1 : cap;
     return (int)c;
 }
 
@@ -131,15 +147,24 @@ __global__ void symcon_bwd_w_partial_kernel(const float *__restrict__ A, const i
     }
 }
 
-__global__ void symcon_bwd_w_reduce_kernel(const float *__restrict__ partial, int total, int n_chunks, float *__restrict__ dW)
+// dW[i] = sum over the chunks of partial[chunk][i]: block = 32 outputs x 32 chunk lanes; lane y adds chunks y, y+32, ... in ascending
+// order, the 32 lane sums are added in lane order (fixed order: deterministic)
+__global__ void __launch_bounds__(1024) symcon_bwd_w_reduce_kernel(const float *__restrict__ partial, int total, int n_chunks, float *__restrict__ dW)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= total) return;
+    __shared__ float part[32][33];
+    const int i = blockIdx.x * 32 + threadIdx.x;
     float acc = 0.0f;
-    for (int c = 0; c < n_chunks; ++c) acc += partial[(size_t)c * total + i];
-    dW[i] = acc;
+    if (i < total)
+        for (int c = threadIdx.y; c < n_chunks; c += 32) acc += partial[(size_t)c * total + i];
+    part[threadIdx.y][threadIdx.x] = acc;
+    __syncthreads();
+    if (threadIdx.y == 0 && i < total) {
+        float t = 0.0f;
+#pragma unroll
+        for (int y = 0; y < 32; ++y) t += part[y][threadIdx.x];
+        dW[i] = t;
+    }
 }
-
 
 // ---------------------------------------------------------------------------------------------------------------------
 // Run-time specialisation (same idea as the tensor-product kernels): one thread = one (node, channel); the node's input rows
@@ -257,35 +282,59 @@ std::string gen_symcon_source(const std::vector<ScTerm> &ts, int in_dim, int out
     o.f("  float *da = dA + (size_t)n * IN * C + u;\n");
     for (int r = 0; r < in_dim; ++r) o.f("  da[(size_t)%d * C] = d%d;\n", r, r);
     o.f("}\n\n");
-    // ---- grad_weights partial sums
-    o.f("extern \"C\" __global__ void __launch_bounds__(128) e3_sc_bwd_w(const float *__restrict__ A, const int *__restrict__ species, const float *__restrict__ G,\n"
-        "    int N, int C, int n_species, int n_chunks, float *__restrict__ partial)\n{\n"
-        "  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;\n  if (idx >= (long long)n_chunks * C) return;\n"
-        "  const int chunk = (int)(idx / C), u = (int)(idx - (long long)chunk * C);\n"
-        "  const int per = (N + n_chunks - 1) / n_chunks;\n  const int n0 = min(N, chunk * per), n1 = min(N, n0 + per);\n"
-        "  float *dst = partial + (size_t)chunk * n_species * NP * C + u;\n"
-        "  for (int i = 0; i < n_species * NP; ++i) dst[(size_t)i * C] = 0.0f;\n"
-        "#pragma unroll 1\n  for (int n = n0; n < n1; ++n) {\n"
-        "    const float *a = A + (size_t)n * IN * C + u, *g = G + (size_t)n * OUT * C + u;\n");
-    for (int r = 0; r < in_dim; ++r) o.f("    const float x%d = a[(size_t)%d * C];\n", r, r);
-    o.f("    int z = species[n]; z = z < 0 ? 0 : (z >= n_species ? n_species - 1 : z);\n    float *dz = dst + (size_t)z * NP * C;\n");
-    {
-        std::map<std::pair<int, int>, int> seen;
-        int tmp = 0;
-        for (int p = 0; p < n_paths; ++p) {
-            std::string total;
-            for (auto &q : rp) {
-                if (q.second != p) continue;
-                const std::string sum = sc_row_sum(o, seen, ts, q.first, p, "    ", tmp);
-                const std::string nm = "s" + std::to_string(tmp++);
-                if (total.empty()) o.f("    const float %s = g[(size_t)%d * C] * %s;\n", nm.c_str(), q.first, sum.c_str());
-                else o.f("    const float %s = fmaf(g[(size_t)%d * C], %s, %s);\n", nm.c_str(), q.first, sum.c_str(), total.c_str());
-                total = nm;
-            }
-            if (!total.empty()) o.f("    dz[(size_t)%d * C] += %s;\n", p, total.c_str());
+    // ---- node-chunk kernels: thread = (chunk, channel) walks the chunk's nodes in ascending order; the grad_weights contributions
+    // s_p = sum_R g[R] * (row sum) are added to per-thread accumulators [species][path] in shared memory (column threadIdx.x of a
+    // [n_species * NP][128] array: no bank conflicts, no sharing between threads) and written out once per chunk.  e3_sc_bwd_w does only
+    // that; e3_sc_bwd_both also forms the node's grad_feats rows (same statements, same order as e3_sc_bwd_feats), so that a VJP call
+    // that wants both gradients reads feats and grad_out once.
+    for (int both = 0; both < 2; ++both) {
+        o.f("extern \"C\" __global__ void __launch_bounds__(128) %s(const float *__restrict__ A, const int *__restrict__ species, const float *__restrict__ W,\n"
+            "    const float *__restrict__ G, int N, int C, int n_species, int n_chunks, float *__restrict__ dA, float *__restrict__ partial)\n{\n",
+            both ? "e3_sc_bwd_both" : "e3_sc_bwd_w");
+        o.s += "  extern __shared__ float acc[];\n"
+               "  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;\n  if (idx >= (long long)n_chunks * C) return;\n"
+               "  const int chunk = (int)(idx / C), u = (int)(idx - (long long)chunk * C);\n"
+               "  const int per = (N + n_chunks - 1) / n_chunks;\n  const int n0 = min(N, chunk * per), n1 = min(N, n0 + per);\n"
+               "  float *my = acc + threadIdx.x;\n  const int nacc = n_species * NP;\n"
+               "  for (int i = 0; i < nacc; ++i) my[i * 128] = 0.0f;\n"
+               "#pragma unroll 1\n  for (int n = n0; n < n1; ++n) {\n"
+               "    const float *a = A + (size_t)n * IN * C + u, *g = G + (size_t)n * OUT * C + u;\n";
+        for (int r = 0; r < in_dim; ++r) o.f(both ? "    const float x%d = a[(size_t)%d * C]; float d%d = 0.0f;\n" : "    const float x%d = a[(size_t)%d * C];\n", r, r, r);
+        o.f("    int z = species[n]; z = z < 0 ? 0 : (z >= n_species ? n_species - 1 : z);\n    float *mz = my + z * NP * 128;\n");
+        if (both) {
+            o.f("    const float *w = W + (size_t)z * NP * C + u;\n");
+            for (int p = 0; p < n_paths; ++p) o.f("    const float w%d = w[(size_t)%d * C];\n", p, p);
         }
+        std::map<std::pair<int, int>, int> seen;
+        std::vector<std::string> cur(n_paths);
+        int tmp = 0, k = 0;
+        for (auto &q : rp) {                                           // row-major, as in e3_sc_bwd_feats; per path the rows ascend
+            o.f("    const float g%d = g[(size_t)%d * C];\n", k, q.first);
+            const std::string sum = sc_row_sum(o, seen, ts, q.first, q.second, "    ", tmp);
+            const std::string nm = "s" + std::to_string(tmp++);
+            if (cur[q.second].empty()) o.f("    const float %s = g%d * %s;\n", nm.c_str(), k, sum.c_str());
+            else o.f("    const float %s = fmaf(g%d, %s, %s);\n", nm.c_str(), k, sum.c_str(), cur[q.second].c_str());
+            cur[q.second] = nm;
+            if (both) {
+                o.f("    { const float gw = w%d * g%d;\n", q.second, k);
+                for (const ScTerm &t : ts) {
+                    if (t.grow != q.first || t.p != q.second) continue;
+                    if (t.a2 < 0) { o.f("      d%d = fmaf(%s, gw, d%d);\n", t.a1, fimm(t.c).c_str(), t.a1); continue; }
+                    o.f("      { const float cg = %s * gw; d%d = fmaf(cg, x%d, d%d); d%d = fmaf(cg, x%d, d%d); }\n", fimm(t.c).c_str(), t.a1, t.a2, t.a1, t.a2, t.a1, t.a2);
+                }
+                o.f("    }\n");
+            }
+            ++k;
+        }
+        for (int p = 0; p < n_paths; ++p)
+            if (!cur[p].empty()) o.f("    mz[%d * 128] += %s;\n", p, cur[p].c_str());
+        if (both) {
+            o.f("    float *da = dA + (size_t)n * IN * C + u;\n");
+            for (int r = 0; r < in_dim; ++r) o.f("    da[(size_t)%d * C] = d%d;\n", r, r);
+        }
+        o.s += "  }\n  float *dst = partial + (size_t)chunk * nacc * C + u;\n"
+               "  for (int i = 0; i < nacc; ++i) dst[(size_t)i * C] = my[i * 128];\n}\n\n";
     }
-    o.f("  }\n}\n");
     return o.s;
 }
 
@@ -305,7 +354,7 @@ extern "C" int e3_symcon_destroy(e3_symcon *sc)
     if (!sc) return E3_OK;
     void *ptrs[] = { sc->f_ptr, sc->f_a1, sc->f_a2, sc->f_p, sc->f_c, sc->b_ptr, sc->b_other, sc->b_g, sc->b_p, sc->b_c, sc->w_ptr, sc->w_a1, sc->w_a2, sc->w_g, sc->w_c };
     for (void *p : ptrs) if (p) cudaFree(p);
-    jit_unload(sc->jfwd); jit_unload(sc->jbf); jit_unload(sc->jbw);
+    jit_unload(sc->jfwd); jit_unload(sc->jbf); jit_unload(sc->jbw); jit_unload(sc->jbb);
     delete sc;
     return E3_OK;
 }
@@ -432,11 +481,30 @@ static int symcon_create_impl(e3_symcon **out, const e3_irrep *irreps_in, int n_
         if (rc == E3_OK) {
             sc->jbf = sc->jfwd; sc->jbf.name = "e3_sc_bwd_feats"; sc->jbf.lib = nullptr; sc->jbf.fn = nullptr;
             sc->jbw = sc->jfwd; sc->jbw.name = "e3_sc_bwd_w"; sc->jbw.lib = nullptr; sc->jbw.fn = nullptr;
+            sc->jbb = sc->jfwd; sc->jbb.name = "e3_sc_bwd_both"; sc->jbb.lib = nullptr; sc->jbb.fn = nullptr;
             if (regs) *regs = sc->jfwd.regs;
             if (spill) *spill = sc->jfwd.spill;
             if (device) rc = jit_load(sc->jfwd);
             if (device && rc == E3_OK) rc = jit_load(sc->jbf);
             if (device && rc == E3_OK) rc = jit_load(sc->jbw);
+            if (device && rc == E3_OK) rc = jit_load(sc->jbb);
+            if (device && rc == E3_OK) {        // shared accumulators of the node-chunk kernels: [n_species * n_paths][128] floats
+                const long long need = (long long)n_species * n_paths * 128 * (long long)sizeof(float);
+                if (need <= 200 * 1024) {
+                    sc->acc_smem = (int)need;
+                    if (need > 48 * 1024) {
+                        cudaError_t e = cudaFuncSetAttribute((const void *)sc->jbw.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)need);
+                        if (e == cudaSuccess) e = cudaFuncSetAttribute((const void *)sc->jbb.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)need);
+                        if (e != cudaSuccess) rc = cuda_fail(e, "cudaFuncSetAttribute(symmetric contraction accumulators)");
+                    }
+                    int dev = 0, nsm = 0, occ = 0;
+                    cudaGetDevice(&dev);
+                    if (rc == E3_OK && cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess &&
+                        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)sc->jbb.fn, 128, (size_t)need) == cudaSuccess && nsm > 0 && occ > 0)
+                        sc->slots = nsm * occ;
+                    cudaGetLastError();
+                }
+            }
             sc->jit = device && rc == E3_OK;
         }
     }
@@ -493,7 +561,7 @@ extern "C" size_t e3_symcon_workspace_bytes(const e3_symcon *sc, int32_t n_nodes
 {
     if (!sc) return 0;
     const long long per = (long long)sc->n_species * sc->n_paths * sc->C;
-    return (size_t)symcon_chunks(n_nodes, per) * per * sizeof(float) + 256;
+    return (size_t)symcon_chunks(n_nodes, sc->C, per, sc->slots) * per * sizeof(float) + 256;
 }
 
 extern "C" int e3_symcon_bwd(const e3_symcon *sc, const float *feats, const int32_t *species, const float *weights, int32_t n_nodes, const float *grad_out,
@@ -504,18 +572,28 @@ extern "C" int e3_symcon_bwd(const e3_symcon *sc, const float *feats, const int3
     if (sc->jit) {
         long long NC = (long long)n_nodes * sc->C;
         int C = sc->C, ns = sc->n_species, N = n_nodes;
-        if (grad_feats && n_nodes > 0) {
+        const int total = sc->n_species * sc->n_paths * sc->C;
+        int chunks = symcon_chunks(n_nodes, sc->C, total, sc->slots);
+        float *partial = reinterpret_cast<float *>(workspace);
+        if (grad_weights && (!workspace || workspace_bytes < e3_symcon_workspace_bytes(sc, n_nodes))) { set_error("e3_symcon_bwd: workspace too small"); return E3_ERR_WORKSPACE; }
+        const bool chunk_kernels = grad_weights && sc->acc_smem > 0 && n_nodes > 0;
+        if (grad_feats && n_nodes > 0 && !chunk_kernels) {
             void *args[] = { (void *)&feats, (void *)&species, (void *)&weights, (void *)&grad_out, (void *)&NC, (void *)&C, (void *)&ns, (void *)&grad_feats };
             E3_CUDA_TRY(cudaLaunchKernel((const void *)sc->jbf.fn, dim3((unsigned)((NC + 127) / 128)), dim3(128), args, 0, st));
         }
+        if (chunk_kernels) {           // one pass over feats and grad_out for both gradients (or for grad_weights alone)
+            void *args[] = { (void *)&feats, (void *)&species, (void *)&weights, (void *)&grad_out, (void *)&N, (void *)&C, (void *)&ns, (void *)&chunks,
+                             (void *)&grad_feats, (void *)&partial };
+            const cudaKernel_t fn = grad_feats ? sc->jbb.fn : sc->jbw.fn;
+            E3_CUDA_TRY(cudaLaunchKernel((const void *)fn, dim3((unsigned)(((long long)chunks * C + 127) / 128)), dim3(128), args, (size_t)sc->acc_smem, st));
+        } else if (grad_weights) {     // accumulators too large for shared memory (or no nodes): table-driven partial sums
+            const int pc = sc->n_paths * sc->C;
+            symcon_bwd_w_partial_kernel<<<dim3((unsigned)chunks, (unsigned)((pc + 127) / 128)), 128, 0, st>>>(
+                feats, species, grad_out, sc->C, sc->in_dim, sc->out_dim, sc->n_paths, sc->n_species, n_nodes, chunks, sc->w_ptr, sc->w_a1, sc->w_a2, sc->w_g, sc->w_c, partial);
+            E3_CUDA_TRY(cudaGetLastError());
+        }
         if (grad_weights) {
-            if (!workspace || workspace_bytes < e3_symcon_workspace_bytes(sc, n_nodes)) { set_error("e3_symcon_bwd: workspace too small"); return E3_ERR_WORKSPACE; }
-            float *partial = reinterpret_cast<float *>(workspace);
-            const int total = sc->n_species * sc->n_paths * sc->C;
-            int chunks = symcon_chunks(n_nodes, total);
-            void *args[] = { (void *)&feats, (void *)&species, (void *)&grad_out, (void *)&N, (void *)&C, (void *)&ns, (void *)&chunks, (void *)&partial };
-            E3_CUDA_TRY(cudaLaunchKernel((const void *)sc->jbw.fn, dim3((unsigned)(((long long)chunks * C + 127) / 128)), dim3(128), args, 0, st));
-            symcon_bwd_w_reduce_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(partial, total, chunks, grad_weights);
+            symcon_bwd_w_reduce_kernel<<<(unsigned)((total + 31) / 32), dim3(32, 32), 0, st>>>(partial, total, chunks, grad_weights);
             E3_CUDA_TRY(cudaGetLastError());
         }
         return E3_OK;
@@ -535,11 +613,11 @@ extern "C" int e3_symcon_bwd(const e3_symcon *sc, const float *feats, const int3
     if (grad_weights) {
         if (!workspace || workspace_bytes < e3_symcon_workspace_bytes(sc, n_nodes)) { set_error("e3_symcon_bwd: workspace too small"); return E3_ERR_WORKSPACE; }
         float *partial = reinterpret_cast<float *>(workspace);
-        const int pc = sc->n_paths * sc->C, total = sc->n_species * pc, chunks = symcon_chunks(n_nodes, total);
+        const int pc = sc->n_paths * sc->C, total = sc->n_species * pc, chunks = symcon_chunks(n_nodes, sc->C, total, sc->slots);
         symcon_bwd_w_partial_kernel<<<dim3((unsigned)chunks, (unsigned)((pc + 127) / 128)), 128, 0, st>>>(
             feats, species, grad_out, sc->C, sc->in_dim, sc->out_dim, sc->n_paths, sc->n_species, n_nodes, chunks, sc->w_ptr, sc->w_a1, sc->w_a2, sc->w_g, sc->w_c, partial);
         E3_CUDA_TRY(cudaGetLastError());
-        symcon_bwd_w_reduce_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(partial, total, chunks, grad_weights);
+        symcon_bwd_w_reduce_kernel<<<(unsigned)((total + 31) / 32), dim3(32, 32), 0, st>>>(partial, total, chunks, grad_weights);
         E3_CUDA_TRY(cudaGetLastError());
     }
     return E3_OK;

@@ -11,7 +11,9 @@ pytestmark = pytest.mark.gpu
 
 
 @pytest.mark.parametrize("C,lmax,out_lmax,N,S,natural", [(128, 3, 2, 1536, 4, True), (64, 2, 2, 700, 10, True), (33, 1, 1, 50, 1, False),
-                                                          (8, 3, 3, 5, 3, False), (256, 2, 1, 64, 2, True)])
+                                                          (8, 3, 3, 5, 3, False), (256, 2, 1, 64, 2, True),
+                                                          (32, 3, 3, 300, 30, False),       # [species][path] accumulators too large for shared memory
+                                                          (128, 3, 3, 20000, 4, True)])     # several waves of node chunks
 @pytest.mark.parametrize("jit", [True, False])
 def test_symmetric_contraction_against_oracle(C, lmax, out_lmax, N, S, natural, jit, monkeypatch):
     """Both kernel families: the run-time specialised ones (default) and the table-driven fallback (E3_SYMCON_JIT=0)."""
