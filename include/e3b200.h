@@ -281,7 +281,8 @@ int e3_sh_bwd_bwd(const e3_plan *plan, const float *vec, const float *grad_sh, c
  * [0, n_species) (values outside are clamped, never read out of bounds).  e3_symcon_bwd returns grad_feats [N,in_dim*C] and
  * grad_weights [n_species,n_paths,C] (either may be NULL) for grad_out = dL/d out; workspace >= e3_symcon_workspace_bytes is needed
  * for grad_weights.  Deterministic (every element is summed by one thread in a fixed order; grad_weights over node chunks -- their
- * number depends on n_nodes only -- in chunk order).  The kernels are specialised for the path table at creation (NVRTC; E3_SYMCON_JIT=0
+ * number depends on n_nodes, C, the table sizes and the device type only -- in a fixed order).  A call that wants both gradients reads feats and
+ * grad_out once (one combined kernel); its results are bit-identical to those of the single-gradient calls.  The kernels are specialised for the path table at creation (NVRTC; E3_SYMCON_JIT=0
  * keeps the table-driven fallback, which is also used beyond 6000 CG terms).  e3_symcon_create needs a device (the CG tensors come from the planner kernel) and synchronises.
  * -------------------------------------------------------------------------------------------*/
 typedef struct e3_symcon e3_symcon;

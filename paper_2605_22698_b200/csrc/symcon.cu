@@ -46,16 +46,17 @@ struct e3_symcon {
 
 namespace {
 
-// node chunks of the grad_weights partial sums: a thread (chunk, channel) walks its chunk's nodes serially.  About 32 nodes per chunk; for
-// small N fewer (down to 4) so that the launch still covers the machine; the number of 128-thread CTAs is rounded up to whole waves of
-// `slots` resident CTAs (equal-length CTAs: a partial last wave costs a whole one); at most 256 MB of partial sums.  A function of
-// (N, C, table sizes, device) only: the summation order is fixed for a given problem on a given device type.
+// node chunks of the grad_weights partial sums: a thread (chunk, channel) walks its chunk's nodes serially.  At most 128 nodes per chunk;
+// the number of 128-thread CTAs is rounded up to whole waves of `slots` resident CTAs (equal-length CTAs: a partial last wave costs a
+// whole one; measured on 100 000 nodes x 64 channels: one wave of 85-node chunks 0.50 ms, three waves of 29-node chunks 0.52, five of 15
+// 0.54); small problems get shorter chunks (down to 4 nodes) so that the launch still covers the machine; at most 256 MB of partial
+// sums.  A function of (N, C, table sizes, device) only: the summation order is fixed for a given problem on a given device type.
 static int symcon_chunks(long long N, long long C, long long per_chunk_floats, long long slots)
 {
     if (N <= 0) return 1;
     if (C < 1) C = 1;
     if (slots < 1) slots = 592;
-    long long c = (N + 31) / 32;
+    long long c = (N + 127) / 128;
     long long ctas = (c * C + 127) / 128;
     if (ctas < slots) {                                   // small problem: shorter chunks, one wave at most
         const long long c4 = (N + 3) / 4, ctas4 = (c4 * C + 127) / 128;
@@ -288,7 +289,7 @@ std::string gen_symcon_source(const std::vector<ScTerm> &ts, int in_dim, int out
     // that; e3_sc_bwd_both also forms the node's grad_feats rows (same statements, same order as e3_sc_bwd_feats), so that a VJP call
     // that wants both gradients reads feats and grad_out once.
     for (int both = 0; both < 2; ++both) {
-        o.f("extern \"C\" __global__ void __launch_bounds__(128) %s(const float *__restrict__ A, const int *__restrict__ species, const float *__restrict__ W,\n"
+        o.f("extern \"C\" __global__ void __launch_bounds__(128, 4) %s(const float *__restrict__ A, const int *__restrict__ species, const float *__restrict__ W,\n"
             "    const float *__restrict__ G, int N, int C, int n_species, int n_chunks, float *__restrict__ dA, float *__restrict__ partial)\n{\n",
             both ? "e3_sc_bwd_both" : "e3_sc_bwd_w");
         o.s += "  extern __shared__ float acc[];\n"
