@@ -638,6 +638,165 @@ __global__ void __launch_bounds__(256, MINB) radial_gemm_bwd_kernel(const float 
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem), "n"(64 * kBwdTiles) : "memory");
 }
 
+// BACKWARD, warp-specialised version of the kernel above: NG groups of four producer warps and one MMA-issuing warp.  Group g owns
+// shared-memory stage g and the K chunks kc = g (mod NG): it loads its chunk of grad_weights (and of W3) into registers, waits until
+// the MMAs of its previous chunk have left the stage (empty[g], tcgen05.commit), splits and stores the chunk, fences the async proxy,
+// arrives on full[g] (128 arrivals) and at once issues the loads of its next chunk; the MMA warp waits for full[g] chunk after chunk
+// and issues the three products.  No block-wide barrier in the loop.
+// What made the difference is the LANE MAPPING of the global loads (ncu on the lock-step kernel: L1 data-pipe LSU wavefronts at 96 %
+// of peak, DRAM at 31 %): a 128-bit load is served a quarter-warp at a time, and with lanes 0-7 on eight different rows every quarter
+// touched eight 128-byte lines -- 32 wavefronts per warp load.  Here consecutive lanes read consecutive 16-byte quads of ONE row
+// (4 lanes x 64 bytes for KC = 16, 8 lanes x 128 bytes for KC = 32), so a quarter-warp touches two lines (one).  To keep the
+// shared-memory stores of that mapping conflict-free the canonical layout is PADDED: core matrices (8 rows x 16 bytes) are LBO = 160
+// (144) bytes apart along K instead of 128, so that the quads of a row fall into different 16-byte bank groups.
+template <int LBO, int SBO>
+__device__ __forceinline__ uint64_t umma_desc_pad(uint32_t smem_addr)
+{
+    uint64_t d = 0;
+    d |= (uint64_t)((smem_addr >> 4) & 0x3fff);
+    d |= (uint64_t)(((uint32_t)LBO >> 4) & 0x3fff) << 16;
+    d |= (uint64_t)(((uint32_t)SBO >> 4) & 0x3fff) << 32;
+    d |= (uint64_t)1 << 46;
+    return d;
+}
+template <int KS, int LBO, int SBO>
+__device__ __forceinline__ void issue_chunk_pad(uint32_t tmem_d, uint32_t sAhi, uint32_t sAlo, uint32_t sBhi, uint32_t sBlo, uint32_t idesc, bool first)
+{
+#pragma unroll
+    for (int ks = 0; ks < KS; ++ks) {
+        const uint64_t ahi = umma_desc_pad<LBO, SBO>(sAhi + ks * 2 * LBO), alo = umma_desc_pad<LBO, SBO>(sAlo + ks * 2 * LBO);
+        const uint64_t bhi = umma_desc_pad<LBO, SBO>(sBhi + ks * 2 * LBO), blo = umma_desc_pad<LBO, SBO>(sBlo + ks * 2 * LBO);
+        const uint32_t acc0 = (!first || ks > 0) ? 1u : 0u;
+        asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}"
+                     :: "r"(tmem_d), "l"(alo), "l"(bhi), "r"(idesc), "r"(acc0) : "memory");
+        asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}"
+                     :: "r"(tmem_d), "l"(ahi), "l"(blo), "r"(idesc), "r"(1u) : "memory");
+        asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}"
+                     :: "r"(tmem_d), "l"(ahi), "l"(bhi), "r"(idesc), "r"(1u) : "memory");
+    }
+}
+
+template <int NT, int KC, int NG>
+__global__ void __launch_bounds__(128 * NG + 32, 1) radial_gemm_bwd_pp_kernel(const float *__restrict__ A, long long lda, const float *__restrict__ Bhi,
+                                                                            const float *__restrict__ Blo, long long ldb, float *__restrict__ D, long long M, long long Kt, int dbg)
+{
+    constexpr int kRows = 128 * NT;
+    constexpr int kQPR = KC / 4;                                       // 16-byte quads per row of a chunk = lanes per row (4 or 8)
+    static_assert(kQPR == 4 || kQPR == 8, "KC must be 16 or 32");
+    constexpr int kLBO = kQPR == 4 ? 160 : 144;                        // padded K stride of the core matrices (see above)
+    constexpr int kSBO = kQPR * kLBO;                                  // bytes between groups of 8 rows
+    constexpr int kPlane = (kRows / 8) * kSBO, kB = 8 * kSBO;
+    constexpr int kStage = 2 * kPlane + 2 * kB;                        // A hi | A lo | B hi | B lo
+    constexpr int kRPI = 32 / kQPR;                                    // rows per warp instruction (8 or 4)
+    constexpr int kRPP = 4 * kRPI;                                     // rows per pass of a four-warp group (32 or 16)
+    constexpr int kPA = kRows / kRPP, kPB = 64 / kRPP;                 // 16-byte pieces of A / of each B plane per producer thread and chunk
+    extern __shared__ __align__(1024) unsigned char smem[];
+    __shared__ __align__(8) unsigned long long mbar[2 * NG + 1];       // full[NG], empty[NG], done
+    __shared__ uint32_t tmem_base_s;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const long long m0 = (long long)blockIdx.x * kRows;
+    const uint32_t mbar_s = (uint32_t)__cvta_generic_to_shared(&mbar[0]);
+    const uint32_t full_s = mbar_s, empty_s = mbar_s + 8 * NG, done_s = mbar_s + 16 * NG;
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"((uint32_t)__cvta_generic_to_shared(&tmem_base_s)), "n"(64 * NT) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    if (tid == 0) {
+        for (int g = 0; g < NG; ++g) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 128;" :: "r"(full_s + 8 * g) : "memory");
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(empty_s + 8 * g) : "memory");
+        }
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(done_s) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem = tmem_base_s;
+    const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(kH >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
+    const uint32_t smem_s = (uint32_t)__cvta_generic_to_shared(smem);
+    const int k_chunks = (int)((Kt + KC - 1) / KC);
+    if (warp == 4 * NG) {
+        if (lane == 0) {
+            for (int kc = 0; kc < k_chunks; ++kc) {
+                const int g = kc % NG;
+                mbar_wait_parity(full_s + 8 * g, (uint32_t)((kc / NG) & 1));
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const uint32_t b = smem_s + g * kStage;
+#pragma unroll
+                for (int t = 0; t < NT; ++t)
+                    if ((t == 0 || m0 + t * kTileM < M) && !(dbg & 8))
+                        issue_chunk_pad<KC / 8, kLBO, kSBO>(tmem + 64 * t, b + t * 16 * kSBO, b + kPlane + t * 16 * kSBO, b + 2 * kPlane, b + 2 * kPlane + kB, idesc, kc == 0);
+                asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(empty_s + 8 * g) : "memory");
+            }
+            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(done_s) : "memory");
+        }
+    } else {
+        const int g = warp >> 2;
+        const int rl = (warp & 3) * kRPI + lane / kQPR, ql = lane % kQPR;          // row within a pass, quad within the row
+        const uint32_t off0 = (uint32_t)((rl >> 3) * kSBO + ql * kLBO + (rl & 7) * 16);
+        constexpr uint32_t kOffPass = (uint32_t)((kRPP / 8) * kSBO);               // kRPP is a multiple of 8: whole row groups per pass
+        float4 ra[kPA], rbh[kPB], rbl[kPB];
+        auto load_chunk = [&](int kc) {
+            const long long k0 = (long long)kc * KC + ql * 4;
+            const bool kok = k0 + 4 <= Kt;
+#pragma unroll
+            for (int j = 0; j < kPA; ++j) {
+                const long long row = m0 + j * kRPP + rl;
+                ra[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (row < M && kok && !(dbg & 2)) ra[j] = __ldcs(reinterpret_cast<const float4 *>(A + row * lda + k0));
+            }
+#pragma unroll
+            for (int j = 0; j < kPB; ++j) {
+                const int row = j * kRPP + rl;
+                rbh[j] = make_float4(0.f, 0.f, 0.f, 0.f); rbl[j] = rbh[j];
+                if (kok) {
+                    rbh[j] = __ldg(reinterpret_cast<const float4 *>(Bhi + (long long)row * ldb + k0));
+                    rbl[j] = __ldg(reinterpret_cast<const float4 *>(Blo + (long long)row * ldb + k0));
+                }
+            }
+        };
+        unsigned char *base = smem + g * kStage;
+        uint32_t ph = 0;
+        if (g < k_chunks) load_chunk(g);
+        for (int kc = g; kc < k_chunks; kc += NG) {
+            if (kc >= NG) {                              // the MMAs of this group's previous chunk must have finished reading the stage
+                mbar_wait_parity(empty_s + 8 * g, ph);
+                ph ^= 1u;
+            }
+            if (!(dbg & 4)) {
+#pragma unroll
+                for (int j = 0; j < kPA; ++j) {
+                    const float4 v = ra[j];
+                    const float4 h = make_float4(tf32_hi(v.x), tf32_hi(v.y), tf32_hi(v.z), tf32_hi(v.w));
+                    const uint32_t off = off0 + j * kOffPass;
+                    *reinterpret_cast<float4 *>(base + off) = h;
+                    *reinterpret_cast<float4 *>(base + kPlane + off) = make_float4(v.x - h.x, v.y - h.y, v.z - h.z, v.w - h.w);
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < kPB; ++j) {
+                const uint32_t off = off0 + j * kOffPass;
+                *reinterpret_cast<float4 *>(base + 2 * kPlane + off) = rbh[j];
+                *reinterpret_cast<float4 *>(base + 2 * kPlane + kB + off) = rbl[j];
+            }
+            if (!(dbg & 1)) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(full_s + 8 * g) : "memory");
+            if (kc + NG < k_chunks) load_chunk(kc + NG);
+        }
+        mbar_wait_parity(done_s, 0u);                   // every MMA has finished: accumulators complete, all stages free
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        if (warp < 8) {
+            float *stg = reinterpret_cast<float *>(smem);
+            for (int t = 0; t < NT; ++t)
+                if (t == 0 || m0 + t * kTileM < M) epilogue_tile<kH>(tmem + 64 * t, warp, lane, stg, D, kH, m0 + t * kTileM, M, 0, kH);
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem), "n"(64 * NT) : "memory");
+}
+
 constexpr int kGemmSmemFwd = 229376;   // forward: 2 x 64 KB of A + 3 x 32 KB of B
 constexpr int kGemmSmem = 196608;      //; backward: 2 x 96 KB stages (the epilogue stages through an idle buffer)
 
@@ -682,6 +841,24 @@ int launch_gemm_bwd(const float *A, long long lda, const float *Bhi, const float
     const long long grid = (M + 128 * nt - 1) / (128 * nt);
     if (grid > 0x7fffffffLL) { set_error("radial gemm: grid too large"); return E3_ERR_UNSUPPORTED; }
     static const int dbg = []() { const char *e = getenv("E3_RADIAL_DBG_BWD"); return e ? atoi(e) : 0; }();
+    static const int pp = []() { const char *e = getenv("E3_RADIAL_BWD_PP"); return e ? atoi(e) : 1; }();      // 0 = the lock-step kernel above
+    if (pp) {
+        constexpr int kPPSmem = 2 * 92160;       // two padded stages (either shape)
+        static bool pp_attr = false;
+        if (!pp_attr) {
+            E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_pp_kernel<4, 16, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPPSmem));
+            E3_CUDA_TRY(cudaFuncSetAttribute(radial_gemm_bwd_pp_kernel<2, 32, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPPSmem));
+            pp_attr = true;
+        }
+        // 256 rows x K chunks of 32 (a row's 128-byte line per chunk) everywhere: config 4 18.2 ms against 19.4 for 512 x 16, config 2 0.284
+        // against 0.363 (whole radial backward); E3_RADIAL_BWD_PP=16 selects the 512 x 16 shape, =0 the lock-step kernel (measurement aids)
+        const bool wide = pp != 16;
+        const long long grid2 = wide ? (M + 255) / 256 : (M + 511) / 512;
+        if (!wide) radial_gemm_bwd_pp_kernel<4, 16, 2><<<(unsigned)grid2, 288, kPPSmem, st>>>(A, lda, Bhi, Blo, ldb, D, M, Kt, dbg);
+        else radial_gemm_bwd_pp_kernel<2, 32, 2><<<(unsigned)grid2, 288, kPPSmem, st>>>(A, lda, Bhi, Blo, ldb, D, M, Kt, dbg);
+        E3_CUDA_TRY(cudaGetLastError());
+        return E3_OK;
+    }
     if (nt == 4) radial_gemm_bwd_kernel<4, 16, 1><<<(unsigned)grid, 256, kGemmSmem, st>>>(A, lda, Bhi, Blo, ldb, D, M, Kt, dbg);
     else radial_gemm_bwd_kernel<2, 32, 1><<<(unsigned)grid, 256, kGemmSmem, st>>>(A, lda, Bhi, Blo, ldb, D, M, Kt, dbg);
     E3_CUDA_TRY(cudaGetLastError());
