@@ -97,3 +97,17 @@ def test_whole_path_with_generated_weights(k):
     assert max(errs[a] for a in ("dx", "dw", "dvec", "F")) <= TOL_VJP, errs
     assert np.abs(F.cpu().numpy().astype(np.float64).sum(0)).max() <= 1e-3 * np.abs(Fr).max()
     net.destroy()
+
+
+@pytest.mark.parametrize("pp", ["0", "16"])
+def test_other_backward_gemm_kernels_still_match_the_oracle(pp):
+    """E3_RADIAL_BWD_PP selects the lock-step backward GEMM (0) or the 512-row x K=16 shape of the warp-specialised one (16); the library
+    reads it once per process, so the parity cases above are re-run in a child process with it set."""
+    import os, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-m", "pytest", os.path.join(root, "tests", "test_gpu_radial.py"), "-q", "-x", "-m", "gpu",
+                        "-k", "test_radial_weights_and_vjp_against_oracle", "-p", "no:cacheprovider"],
+                       env={**os.environ, "E3_RADIAL_BWD_PP": pp}, cwd=root, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
+    assert "6 passed" in r.stdout, r.stdout[-500:]
+
